@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the channel-flow hot path on B200 (metric: BASELINE.json).
+
+A "step" is one pass of the whole hot path over one synthetic field: one full RK3 step
+(3 x chan_substep = rows a1-a12 of DESIGN.md), one chan_filter_store (a13) and one chan_stats
+accumulate (a14).  ``value`` counts only the 3 substeps' grid points (Mpoint*RK-substeps/s), so the
+filter and statistics time is inside the denominator but earns no credit; ``substep_only`` gives the
+rate of the substeps alone.  Inputs are resident in HBM before the timed region; ``e2e`` repeats the
+measurement through the *_host entry points with pinned host buffers (state in, state + filtered
+database + statistics out, every step).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg4|cfg5|mid|cfg1] [--impl reference]
+
+N > 1 (torchrun): the path does not shard without an exchange step, so ranks run
+independent replicas; value = all ranks' points / max-over-ranks time; scaling "weak".
+``--impl reference`` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Mpoint*RK-substeps/s fp64"
+UNIT = "Mpoint*substeps/s"
+
+# Compulsory HBM traffic of each kernel class in bytes per grid point it processes (
+# one complex field pass = 8 B/point).  The SURVEY groups are the section 8(d) figures.
+BYTES_PER_POINT = {
+    "d1_forward": 16, "derive_down": 48, "derive_up": 40, "zfft_inv": 120, "xfft_prod": 108, "zfft_fwd": 60,
+    "y1": 72, "y2": 100, "y3": 76, "y4": 48, "y5": 48, "stats": 48, "transpose": 16,
+}
+SURVEY_GROUPS = {
+    "K2 z-pad + inverse z-FFT": (["zfft_inv"], 120),
+    "K3 x-FFT . products . x-FFT": (["xfft_prod"], 108),
+    "K4 forward z-FFT + truncate": (["zfft_fwd"], 60),
+    "K5+K1 y-phase": (["y1", "y2", "y3", "y4", "y5", "d1_forward", "derive_down", "derive_up", "mean"], 144),
+}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p))["hbm_gbs"], "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.stop = index, [], threading.Event()
+        self.t = threading.Thread(target=self.run, daemon=True)
+
+    def run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 3 + k and r[3 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": float(self.rows[0][1]), "samples": len(self.rows),
+                "power_w_max": max(float(r[2]) for r in self.rows), "reasons": reasons}
+
+
+def pick_workload(name, free_bytes):
+    from paper_1808_06461_b200 import inputs
+    if name != "auto":
+        return name
+    for cand in ("cfg5", "cfg4", "cfg3"):
+        c = inputs.CONFIGS[cand]
+        F = c["nx"] * c["ny"] * c["nz"] * 8
+        if 15.6 * F + 4e9 < free_bytes:      # workspace (15 fields + chunks) + slack
+            return cand
+    return "mid"
+
+
+def oracle_sample(cfg_name, steps, warmup):
+    """The oracle as it stands on a bounded sample: same ny, mesh, Re, dt, box resolution; nx x nz cut down."""
+    from oracle.channel import ChannelOracle
+    from paper_1808_06461_b200 import inputs
+    c = inputs.config(cfg_name)
+    snx, snz = min(c["nx"], 48), min(c["nz"], 32)
+    cs = inputs.config(cfg_name, nx=snx, nz=snz, lx=c["lx"] * snx / c["nx"], lz=c["lz"] * snz / c["nz"],
+                       cut=(min(c["cut"][0], snx // 2 - 1), min(c["cut"][1], snz // 2 - 1)))
+    v, phi, omy = (t.numpy() for t in inputs.fluctuations(cs))
+    o = ChannelOracle(cs["nx"], cs["ny"], cs["nz"], cs["lx"], cs["lz"], cs["y"], cs["re"], cs["dt"])
+    o.set_state(v, phi, omy, cs["U"], cs["W"])
+    pts = cs["nx"] * cs["ny"] * cs["nz"]
+
+    def one():
+        o.step()
+        o.filter_store(*cs["cut"])
+        o.stats_accumulate()
+
+    for _ in range(warmup):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    dt = time.perf_counter() - t0
+    sample = (f"oracle.ChannelOracle, {steps} x (step + filter_store + stats) on a {snx}x{cs['ny']}x{snz} sub-box of {cfg_name} "
+              f"(same mesh, Re, dt, dx, dz; {pts} points)")
+    return 3 * pts * steps / dt / 1e6, dt / steps * 1e3, sample
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = args.workload if args.workload != "auto" else "cfg4"
+    steps = max(1, min(args.steps, 3))
+    val, ms, sample = oracle_sample(wl, steps, min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": wl, "note": "CPU oracle on a bounded sample"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--workload", default="auto")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as entry
+    entry.build()
+    from paper_1808_06461_b200 import binding, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    W = max(args.warmup, 3)
+    K = max(args.steps, 1)
+
+    free_b, total_b = torch.cuda.mem_get_info(dev)
+    wl = pick_workload(args.workload, free_b)
+    c = inputs.config(wl)
+    npts = c["nx"] * c["ny"] * c["nz"]
+    F = npts * 8
+    kxc, kzc = c["cut"]
+
+    # ---- inputs resident in HBM ---------------------------------------------------------------------
+    v, phi, omy = inputs.fluctuations(c, device=dev)
+    U = torch.from_numpy(c["U"]).to(dev)
+    Wm = torch.from_numpy(c["W"]).to(dev)
+    torch.cuda.empty_cache()
+    ch = binding.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    ws_bytes = ch.workspace_bytes()
+    ch.bind(dev)
+    ch.set_state(v, phi, omy, U, Wm)
+    ch._keep = None
+    fout = torch.empty((10, c["ny"], 2 * kzc + 1, kxc + 1), dtype=torch.complex128, device=dev)
+    stream = ch.stream
+
+    def one_step():
+        ch.step()
+        ch.filter_store(kxc, kzc, fout)
+        ch.stats(binding.STATS_ACCUMULATE)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(W):
+        one_step()
+    barrier()
+    l0 = ch.debug_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ch.debug_profile(True)
+    with ClockSampler(local) as clk:
+        barrier()
+        e0.record(stream)
+        for _ in range(K):
+            one_step()
+        e1.record(stream)
+        barrier()
+    ch.debug_profile(False)
+    ms_total = e0.elapsed_time(e1)
+    prof = ch.debug_profile_read()
+    launches = ch.debug_launch_count() - l0
+    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total_max = float(tmax.item())
+    value = world * 3 * npts * K / (ms_total_max * 1e-3) / 1e6
+    # finite-state check: a blown-up field would make the timing meaningless
+    gv = ch.get_state()[0]
+    finite = bool(torch.isfinite(torch.view_as_real(gv)).all().item())
+    del gv
+
+    # ---- substeps alone -----------------------------------------------------------------------------
+    barrier()
+    e0.record(stream)
+    for _ in range(K):
+        ch.step()
+    e1.record(stream)
+    barrier()
+    ms_sub = e0.elapsed_time(e1)
+    substep_only = {"value": 3 * npts * K / (ms_sub * 1e-3) / 1e6, "unit": UNIT, "ms_per_substep": ms_sub / (3 * K)}
+
+    # ---- roofline of the dominant kernel + SURVEY groups ---------------------------------------------
+    peak, peak_src = measured_peaks()
+    sub_classes = {k: v_ for k, v_ in prof.items() if v_[1] > 0}
+    dom = max((k for k in sub_classes if k in BYTES_PER_POINT), key=lambda k: sub_classes[k][0])
+    dms, dcnt = sub_classes[dom]
+    launches_per_field = dcnt / K          # per step
+    # points one launch processes: y-phase kernels and stats see the whole field; plane kernels one chunk
+    uses = {"zfft_inv": 4, "xfft_prod": 3, "zfft_fwd": 3}.get(dom, None)   # field sweeps per step (3 substeps [+ filter])
+    if dom in ("zfft_inv",):
+        pts_per_launch = npts * 4 / launches_per_field
+    elif dom in ("xfft_prod", "zfft_fwd"):
+        pts_per_launch = npts * 3 / launches_per_field
+    elif dom == "stats":
+        pts_per_launch = npts
+    else:
+        pts_per_launch = npts
+    abytes = BYTES_PER_POINT[dom] * pts_per_launch
+    achieved = abytes / (dms / dcnt * 1e-3) / 1e9
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
+                "avg_launch_ms": dms / dcnt, "share_of_step": dms / ms_total}
+    groups = {}
+    for gname, (classes, bpp) in SURVEY_GROUPS.items():
+        gms = sum(prof[k][0] for k in classes if k in prof)
+        if gms > 0:
+            gb = bpp * npts * 3 * K / (gms * 1e-3) / 1e9     # substep part only: the filter has its own classes
+            groups[gname] = {"ms_per_substep": gms / (3 * K), "survey_bytes_per_point": bpp, "achieved_GBs": gb, "frac": gb / peak}
+    # the zfft_inv class is also used by the filter (one extra sweep per step): scale its group to 4 sweeps
+    if "K2 z-pad + inverse z-FFT" in groups:
+        g = groups["K2 z-pad + inverse z-FFT"]
+        g["achieved_GBs"] *= 4.0 / 3.0
+        g["frac"] *= 4.0 / 3.0
+        g["ms_per_substep"] *= 3.0 / 4.0
+    kernel_ms = {k: {"ms_per_step": v_[0] / K, "launches_per_step": v_[1] / K} for k, v_ in sub_classes.items()}
+
+    # ---- end to end through the host-buffer entry points ---------------------------------------------
+    e2e = None
+    if rank == 0 or world > 1:
+        Ke = max(1, min(args.e2e_steps, K))
+        try:
+            hv = torch.empty(ch.shape, dtype=torch.complex128, pin_memory=True)
+            hp = torch.empty(ch.shape, dtype=torch.complex128, pin_memory=True)
+            ho = torch.empty(ch.shape, dtype=torch.complex128, pin_memory=True)
+            hU = torch.empty(c["ny"], dtype=torch.float64, pin_memory=True)
+            hW = torch.empty(c["ny"], dtype=torch.float64, pin_memory=True)
+            hf = torch.empty(tuple(fout.shape), dtype=torch.complex128, pin_memory=True)
+            ch.get_state_host(hv, hp, ho, hU, hW)
+
+            def e2e_step():
+                ch.set_state_host(hv, hp, ho, hU, hW)
+                ch.step()
+                ch.filter_store_host(kxc, kzc, hf)
+                ch.stats(binding.STATS_ACCUMULATE | binding.STATS_READ)
+                ch.get_state_host(hv, hp, ho, hU, hW)
+
+            e2e_step()
+            barrier()
+            t0 = time.perf_counter()
+            e0.record(stream)
+            for _ in range(Ke):
+                e2e_step()
+            e1.record(stream)
+            barrier()
+            wall = (time.perf_counter() - t0) * 1e3
+            ms_e = max(e0.elapsed_time(e1), wall)       # host-side copies block: take the larger clock
+            te = torch.tensor([ms_e], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            state_b = 3 * F + 2 * c["ny"] * 8
+            e2e = {"value": world * 3 * npts * Ke / (float(te.item()) * 1e-3) / 1e6, "unit": UNIT, "steps": Ke,
+                   "ms_per_step": float(te.item()) / Ke, "h2d_bytes_per_step": state_b,
+                   "d2h_bytes_per_step": state_b + hf.numel() * 16 + 10 * c["ny"] * 8,
+                   "api": "chan_set_state_host + chan_step + chan_filter_store_host + chan_stats(READ) + chan_get_state_host, pinned host buffers"}
+            del hv, hp, ho, hf
+        except RuntimeError as ex:      # pinned allocation refused by the host
+            e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+
+    if world > 1:
+        dist.barrier()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        val, ms, sample = oracle_sample(wl, 1, 0)
+        cpu = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+               "host_cores_available": len(os.sched_getaffinity(0))}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_total_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl, "grid": [c["nx"], c["ny"], c["nz"]], "padded": [3 * c["nx"] // 2, c["ny"], 3 * c["nz"] // 2],
+                   "step": "1 RK3 step (3 chan_substep) + chan_filter_store + chan_stats(ACCUMULATE); value counts the 3 substeps",
+                   "filter_cut": [kxc, kzc], "l2": "inputs larger than L2 (one field = %.2f GB)" % (F / 1e9),
+                   "workspace_GB": ws_bytes / 1e9, "multi_gpu": "replicas only", "state_finite": finite},
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches),
+        "substep_only": substep_only, "roofline": roofline, "roofline_groups": groups, "kernel_ms": kernel_ms,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

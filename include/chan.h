@@ -1,0 +1,140 @@
+/* chan.h -- C ABI of the B200-native channel-flow DNS hot path (arxiv 1808.06461).
+ *
+ * One semi-implicit Runge-Kutta substep of incompressible plane-channel flow (section 2.1,
+ * L61-80: walls at y=+-h, periodic x,z, constant mass flux; (omega_y, lap v) formulation [20];
+ * Fourier x,z with zero-padding dealiasing; seven-point compact finite differences in y; three-substep
+ * low-storage RK [34]) plus the paper's low-storage filter and plane statistics (section 3.1-3.2,
+ * L112, L124: sharp Fourier cutoff, ten variables u_i, u_i u_j, om_i om_i).
+ *
+ * Conventions
+ *  - h = 1; nu = 1/re_tau in the caller's velocity unit (reading R9).
+ *  - Retained modes: p = 0..nx/2-1 (k_x = 2 pi p/lx), z slots s = 0..nz-1 in FFT order
+ *    (q = 0..nz/2-1, slot nz/2 always zero, q = -nz/2+1..-1; k_z = 2 pi q/lz).
+ *  - "LINE layout": complex128 interleaved, [nz][nx/2][ny], y fastest.  This is the layout of every
+ *    field that crosses this ABI unless stated otherwise.
+ *  - "device" pointers are CUDA device memory owned (allocated and freed) by the caller; "host"
+ *    pointers are ordinary host memory.  The library allocates no device memory: tables and scratch
+ *    are carved from the workspace handed to chan_bind().
+ *  - Every call returns 0 (CHAN_OK) or a negative status; nothing is printed, nothing throws.
+ *    Calls enqueue work on the stream given to chan_bind() and return without synchronising, except
+ *    chan_stats(READ), chan_get_scalars() and the *_host entry points, which synchronise that stream.
+ *  - A handle is not thread-safe.  There is NO CPU fallback: without a CUDA device every compute call
+ *    returns CHAN_ECUDA.
+ */
+#ifndef CHAN_H_
+#define CHAN_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHAN_OK        0
+#define CHAN_EINVAL   -1  /* bad sizes, non-monotone y, unsupported FFT length, cutoff out of range, NULL */
+#define CHAN_ENOSPACE -2  /* workspace or output buffer too small                                   */
+#define CHAN_ESTATE   -3  /* wrong call order (not bound, no state, chan_step() mid-step)           */
+#define CHAN_ECUDA    -4  /* a CUDA runtime call or kernel launch failed                            */
+
+typedef struct chan chan_t; /* opaque */
+
+/* nx, nz: Fourier collocation points before the 3/2 padding (even; 3nx/2 and 3nz/2 must factor into
+ * 2,3 only); ny: mesh points including both walls (>= 8).  PAPER.md L80. */
+typedef struct { int nx, ny, nz; } chan_grid_t;
+
+/* lx, lz: periods; y: HOST array of ny strictly increasing mesh points, y[0] = -1, y[ny-1] = +1.
+ * The array is copied.  PAPER.md L61, L80 (the paper's own mesh is not printed: reading R10). */
+typedef struct { double lx, lz; const double* y; } chan_box_t;
+
+/* lhs_halfwidth, rhs_halfwidth: compact stencil half widths, 1..3 (default 3,3 = seven-point, L80).
+ * forcing: 0 = constant mass flux, 1 = constant pressure gradient (see chan_set_pgrad). */
+typedef struct { int lhs_halfwidth, rhs_halfwidth; int forcing; } chan_opts_t;
+
+/* Build the plan on the host (compact-difference band tables on the given mesh, their factorisations,
+ * wavenumber and twiddle tables, RK constants).  dt is the FULL three-substep step.  opts may be NULL. */
+int chan_create(chan_t** out, const chan_grid_t* grid, const chan_box_t* box, double re_tau, double dt,
+                const chan_opts_t* opts);
+int chan_destroy(chan_t* h);
+
+/* Bytes of device workspace chan_bind() needs (0 if h is NULL). */
+size_t chan_workspace_bytes(const chan_t* h);
+
+/* Adopt caller-owned device memory (256-byte aligned, >= chan_workspace_bytes) and a CUDA stream
+ * (cudaStream_t cast to void*; NULL = default stream).  Uploads the tables. */
+int chan_bind(chan_t* h, void* dev_workspace, size_t bytes, void* cuda_stream);
+
+/* State at a full-step boundary: v^, phi^ = (D2 - k^2) v^, omega_y^ in LINE layout, and the mean
+ * profiles U(y), W(y) (ny doubles each), all DEVICE pointers.  set_state also fixes the mass flux
+ * Q0 = sum_j w_j U_j (trapezoid weights, reading R8), clears the RK history and derives
+ * u, w, omega_x, omega_z (step a1).  The (0,0) mode and the z-Nyquist slot of the inputs are ignored. */
+int chan_set_state(chan_t* h, const void* dev_v, const void* dev_phi, const void* dev_omy,
+                   const double* dev_U, const double* dev_W);
+int chan_get_state(const chan_t* h, void* dev_v, void* dev_phi, void* dev_omy, double* dev_U, double* dev_W);
+
+/* Same through HOST buffers (pageable or pinned): copies host->device into library scratch inside the
+ * call, then behaves like the device versions; get_state_host synchronises before returning. */
+int chan_set_state_host(chan_t* h, const void* host_v, const void* host_phi, const void* host_omy,
+                        const double* host_U, const double* host_W);
+int chan_get_state_host(chan_t* h, void* host_v, void* host_phi, void* host_omy, double* host_U, double* host_W);
+
+/* One RK substep (steps a3-a12, then a1-a2 for the new state); the substep index cycles 0,1,2. */
+int chan_substep(chan_t* h);
+/* Three substeps; CHAN_ESTATE if called mid-step. */
+int chan_step(chan_t* h);
+
+/* Low-storage filter (a13): writes the ten variables u,v,w, uu,uv,uw,vv,vw,ww, om_i om_i
+ * restricted to 0<=p<=kx_cut, |q|<=kz_cut into dev_out[10][ny][2 kz_cut+1][kx_cut+1] complex128
+ * (z rows ordered q = 0..kz_cut, -kz_cut..-1).  Products are formed on the dealiased grid. */
+int chan_filter_store(chan_t* h, int kx_cut, int kz_cut, void* dev_out, size_t out_bytes);
+/* Same with a HOST output buffer (device staging inside the workspace; synchronises). */
+int chan_filter_store_host(chan_t* h, int kx_cut, int kz_cut, void* host_out, size_t out_bytes);
+
+/* Plane statistics (a14): flags is an OR of the values below.  ACCUMULATE adds the ten profiles
+ * <u>,<v>,<w>,<uu>,<uv>,<uw>,<vv>,<vw>,<ww>,<om_i om_i> of the current state to the running sums;
+ * READ copies sums[10][ny] to host_out and the sample count to *nsamples (synchronises); RESET clears. */
+#define CHAN_STATS_ACCUMULATE 1
+#define CHAN_STATS_READ       2
+#define CHAN_STATS_RESET      4
+int chan_stats(chan_t* h, int flags, double* host_out, long long* nsamples);
+
+/* Scalars: out[0] = -dP/dx recovered by the last substep (constant mass flux) or prescribed,
+ * out[1] = mass flux Q0, out[2] = nu dU/dy at y=-1, out[3] = -nu dU/dy at y=+1.  Synchronises. */
+int chan_get_scalars(chan_t* h, double* host_out4);
+int chan_set_pgrad(chan_t* h, double minus_dpdx); /* forcing == 1 only */
+
+const char* chan_strerror(int status);
+
+/* ---- debug / parity / profiling hooks (run one stage on library buffers) ------------------------
+ * Field ids for chan_debug_get_field / chan_debug_set_field (LINE layout, device pointers): */
+enum { CHAN_F_V = 0, CHAN_F_PHI, CHAN_F_OMY, CHAN_F_U, CHAN_F_W, CHAN_F_OMX, CHAN_F_OMZ,
+       CHAN_F_H1, CHAN_F_H2, CHAN_F_H3, CHAN_F_HV_PREV, CHAN_F_HG_PREV, CHAN_F_COUNT };
+int chan_debug_get_field(const chan_t* h, int field, void* dev_out);
+int chan_debug_set_field(chan_t* h, int field, const void* dev_in);
+/* Stages: run on whatever the library buffers currently hold. */
+enum { CHAN_STAGE_DERIVE = 0,   /* a1-a2: state -> u,w,om_x,om_z                                  */
+       CHAN_STAGE_NONLINEAR,    /* a3-a8: u..om_z -> H1,H2,H3                                      */
+       CHAN_STAGE_YSOLVE,       /* a9-a12: H, state, history -> new state, history (uses substep index) */
+       CHAN_STAGE_COUNT };
+int chan_debug_run_stage(chan_t* h, int stage);
+int chan_debug_set_substep_index(chan_t* h, int i);
+/* Copy of the host-computed compact band tables, out[4][ny][7]: A1, B1, A2, B2 (HOST pointer). */
+int chan_debug_get_band_tables(const chan_t* h, double* host_out);
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+long long chan_debug_launch_count(const chan_t* h);
+/* Per-kernel-class device timing with CUDA events on the bound stream (bench.py's roofline object).
+ * chan_debug_profile(h,1) clears and starts recording one event pair around every kernel launch;
+ * chan_debug_profile(h,0) stops; chan_debug_profile_read synchronises and returns, per class, the summed
+ * milliseconds and the number of launches (arrays of CHAN_KC_COUNT entries, HOST pointers). */
+enum { CHAN_KC_D1FWD = 0, CHAN_KC_DERIVE_DOWN, CHAN_KC_DERIVE_UP, CHAN_KC_ZFFT_INV, CHAN_KC_XFFT_PROD, CHAN_KC_ZFFT_FWD,
+       CHAN_KC_MEAN, CHAN_KC_Y1, CHAN_KC_Y2, CHAN_KC_Y3, CHAN_KC_Y4, CHAN_KC_Y5, CHAN_KC_TRANSPOSE,
+       CHAN_KC_FILTER_COPY, CHAN_KC_XFFT_PROD_FILTER, CHAN_KC_ZFFT_FWD_FILTER, CHAN_KC_STATS, CHAN_KC_COUNT };
+int chan_debug_profile(chan_t* h, int enable);
+int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts);
+/* Plain line<->plane transposes (a2/a8) on caller buffers, for roofline timing: n fields of one
+ * [nz][nx/2][ny] <-> [ny][nz][nx/2] complex128 array each. dir 0: line->plane, 1: plane->line. */
+int chan_debug_transpose(chan_t* h, int dir, const void* dev_in, void* dev_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHAN_H_ */

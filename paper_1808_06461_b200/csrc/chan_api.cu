@@ -1,0 +1,546 @@
+// C ABI of libchan (include/chan.h): handle, workspace carving, launch sequences.
+// No device memory is allocated here: everything is carved from the caller's workspace.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/chan.h"
+#include "chan_fftkernels.cuh"
+#include "chan_plan.h"
+#include "chan_ykernels.cuh"
+
+using namespace chn;
+
+namespace {
+constexpr int kThreadsY = 128;
+constexpr size_t kAlign = 256;
+inline size_t up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+}  // namespace
+
+struct chan {
+    Plan P;
+    bool bound = false, have_state = false;
+    int isub = 0;
+    cudaStream_t stream = nullptr;
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    long long launches = 0;
+    long long nsamples = 0;
+    int cuda_err = 0;
+    // sizes
+    size_t F = 0;          // bytes of one complex field
+    long long nm = 0;
+    int pc = 1;            // planes per FFT chunk
+    int Tz = 1;            // k_x columns per z-FFT tile
+    // device pointers (carved)
+    double2 *v, *phi, *omy, *hv, *hg, *u, *w, *ox, *oz;   // plane layout fields
+    double2 *H1, *H2, *H3;                                 // alias u, w, ox
+    double4* fac; double2 *z1, *z2; double *r1, *r2, *r3, *r4; double4* coef;
+    double2 *zpad, *xh;
+    double *U, *W, *H1p, *H3p, *meanwork, *scal, *stats;
+    // tables
+    double* tab[2][4];     // B1, A2, B2, lu1 per orientation
+    double *kx, *kz, *wm, *wp, *wq;
+    double2 *twx, *twz;
+    size_t need = 0;
+    // per-kernel-class CUDA-event profiling (chan_debug_profile)
+    bool prof_on = false;
+    int cur_kc = 0;
+    std::vector<cudaEvent_t> prof_ev;   // pairs
+    std::vector<int> prof_cls;
+};
+
+namespace {
+
+struct Carver {
+    char* base; size_t off = 0;
+    template <typename T> T* take(size_t bytes) { T* p = base ? reinterpret_cast<T*>(base + off) : nullptr; off += up(bytes); return p; }
+};
+
+void choose_tiling(chan_t* h) {
+    const Plan& P = h->P;
+    int T = 16;
+    while (T > 1 && (size_t)P.mz * T * 16 > 112 * 1024) T >>= 1;
+    while (T > 1 && T > P.nxh) T >>= 1;
+    h->Tz = T;
+    const size_t per_plane = (size_t)13 * P.mz * P.nxh * 16;
+    long long pc = (long long)(1536ull * 1024 * 1024 / per_plane);
+    if (pc < 1) pc = 1;
+    if (pc > P.ny) pc = P.ny;
+    h->pc = (int)pc;
+}
+
+// Lays out the workspace; with base == nullptr only measures.
+size_t carve(chan_t* h, char* base) {
+    const Plan& P = h->P;
+    Carver c{base};
+    const size_t F = h->F;
+    h->v = c.take<double2>(F); h->phi = c.take<double2>(F); h->omy = c.take<double2>(F);
+    h->hv = c.take<double2>(F); h->hg = c.take<double2>(F);
+    h->u = c.take<double2>(F); h->w = c.take<double2>(F); h->ox = c.take<double2>(F); h->oz = c.take<double2>(F);
+    h->H1 = h->u; h->H2 = h->w; h->H3 = h->ox;
+    h->fac = c.take<double4>(2 * F);
+    h->z1 = c.take<double2>(F); h->z2 = c.take<double2>(F);
+    h->r1 = c.take<double>(F / 2); h->r2 = c.take<double>(F / 2); h->r3 = c.take<double>(F / 2); h->r4 = c.take<double>(F / 2);
+    h->coef = c.take<double4>((size_t)h->nm * 32);
+    h->zpad = c.take<double2>((size_t)6 * h->pc * P.mz * P.nxh * 16);
+    h->xh = c.take<double2>((size_t)7 * h->pc * P.mz * P.nxh * 16);
+    const size_t ny8 = (size_t)P.ny * 8;
+    h->U = c.take<double>(ny8); h->W = c.take<double>(ny8); h->H1p = c.take<double>(ny8); h->H3p = c.take<double>(ny8);
+    h->meanwork = c.take<double>(ny8 * 8);
+    h->scal = c.take<double>(64);
+    h->stats = c.take<double>((size_t)10 * P.ny * 8);
+    for (int o = 0; o < 2; ++o) for (int k = 0; k < 4; ++k) h->tab[o][k] = c.take<double>(ny8 * 8);
+    h->kx = c.take<double>((size_t)P.nxh * 8); h->kz = c.take<double>((size_t)P.nz * 8);
+    h->wm = c.take<double>(ny8); h->wp = c.take<double>(ny8); h->wq = c.take<double>(ny8);
+    h->twx = c.take<double2>((size_t)P.mx * 16); h->twz = c.take<double2>((size_t)P.mz * 16);
+    return c.off;
+}
+
+bool ck(chan_t* h, cudaError_t e) {
+    if (e != cudaSuccess) { h->cuda_err = (int)e; return false; }
+    return true;
+}
+#define CK(x) do { if (!ck(h, (x))) return CHAN_ECUDA; } while (0)
+void prof_mark(chan_t* h, int kc, bool begin) {
+    if (!h->prof_on) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, h->stream);
+    h->prof_ev.push_back(e);
+    if (begin) h->prof_cls.push_back(kc);
+}
+#define PB(kc) prof_mark(h, (kc), true)
+#define LAUNCHED() do { ++h->launches; prof_mark(h, 0, false); if (!ck(h, cudaGetLastError())) return CHAN_ECUDA; } while (0)
+
+YParams yparams(const chan_t* h) {
+    const Plan& P = h->P;
+    YParams Y;
+    Y.ny = P.ny; Y.nz = P.nz; Y.nxh = P.nxh; Y.nzh = P.nzh; Y.nm = h->nm;
+    for (int o = 0; o < 2; ++o) { Y.t[o].B1 = h->tab[o][0]; Y.t[o].A2 = h->tab[o][1]; Y.t[o].B2 = h->tab[o][2]; Y.t[o].lu1 = h->tab[o][3]; }
+    Y.kx = h->kx; Y.kz = h->kz; Y.wm = h->wm; Y.wp = h->wp;
+    Y.nu = P.nu; Y.dt = P.dt;
+    Y.alpha = P.rk_alpha[h->isub]; Y.beta = P.rk_beta[h->isub]; Y.gamma = P.rk_gamma[h->isub]; Y.zeta = P.rk_zeta[h->isub];
+    return Y;
+}
+
+PlaneParams pparams(const chan_t* h) {
+    const Plan& P = h->P;
+    PlaneParams Q;
+    Q.ny = P.ny; Q.nz = P.nz; Q.nxh = P.nxh; Q.nzh = P.nzh; Q.mx = P.mx; Q.mz = P.mz; Q.nm = h->nm;
+    Q.fx.n = P.mx; Q.fx.npass = (int)P.fx.radix.size(); Q.fx.tw = h->twx;
+    Q.fz.n = P.mz; Q.fz.npass = (int)P.fz.radix.size(); Q.fz.tw = h->twz;
+    for (int i = 0; i < Q.fx.npass; ++i) Q.fx.radix[i] = P.fx.radix[i];
+    for (int i = 0; i < Q.fz.npass; ++i) Q.fz.radix[i] = P.fz.radix[i];
+    return Q;
+}
+
+inline unsigned ygrid(const chan_t* h) { return (unsigned)((h->nm + kThreadsY - 1) / kThreadsY); }
+
+// a1-a2: state -> u, w, om_x, om_z
+int run_derive(chan_t* h) {
+    YParams Y = yparams(h);
+    PB(CHAN_KC_D1FWD); k_d1_forward<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->v, h->z1); LAUNCHED();
+    PB(CHAN_KC_DERIVE_DOWN); k_derive_down<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->z1, h->omy, h->U, h->W, h->u, h->w, h->z2, (double2*)h->fac); LAUNCHED();
+    PB(CHAN_KC_DERIVE_UP); k_derive_up<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->z2, (double2*)h->fac, h->v, h->ox, h->oz); LAUNCHED();
+    return CHAN_OK;
+}
+
+template <int T> int launch_zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
+    const size_t sm = (size_t)Q.mz * T * 16;
+    CK(cudaFuncSetAttribute(k_zfft_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    dim3 g((Q.nxh + T - 1) / T, npl, nf);
+    PB(CHAN_KC_ZFFT_INV); k_zfft_inv<T><<<g, 256, sm, h->stream>>>(Q, in, j0, npl, h->zpad); LAUNCHED();
+    return CHAN_OK;
+}
+template <int T> int launch_zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out,
+                                 double scale, int filt, int kxc, int kzc) {
+    const size_t sm = (size_t)Q.mz * T * 16;
+    CK(cudaFuncSetAttribute(k_zfft_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    dim3 g((pin + T - 1) / T, npl, nf);
+    PB(filt ? CHAN_KC_ZFFT_FWD_FILTER : CHAN_KC_ZFFT_FWD); k_zfft_fwd<T><<<g, 256, sm, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc); LAUNCHED();
+    return CHAN_OK;
+}
+int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
+    switch (h->Tz) {
+        case 16: return launch_zinv<16>(h, Q, in, nf, j0, npl);
+        case 8: return launch_zinv<8>(h, Q, in, nf, j0, npl);
+        case 4: return launch_zinv<4>(h, Q, in, nf, j0, npl);
+        case 2: return launch_zinv<2>(h, Q, in, nf, j0, npl);
+        default: return launch_zinv<1>(h, Q, in, nf, j0, npl);
+    }
+}
+int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out, double scale, int filt, int kxc, int kzc) {
+    switch (h->Tz) {
+        case 16: return launch_zfwd<16>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
+        case 8: return launch_zfwd<8>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
+        case 4: return launch_zfwd<4>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
+        case 2: return launch_zfwd<2>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
+        default: return launch_zfwd<1>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
+    }
+}
+
+// a3-a8 (nprod = 3) or the product part of a13 (nprod = 7)
+int run_planes(chan_t* h, int nprod, const FieldPtrsW& out, int kxc, int kzc) {
+    const Plan& P = h->P;
+    PlaneParams Q = pparams(h);
+    FieldPtrs in;
+    in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w; in.f[3] = h->ox; in.f[4] = h->omy; in.f[5] = h->oz;
+    const int pout = (nprod == 3) ? P.nxh : kxc + 1;
+    const double scale = 1.0 / ((double)P.mx * (double)P.mz);
+    const size_t smx = (size_t)(nprod == 3 ? 3 : 4) * P.mx * 16;
+    if (nprod == 3) CK(cudaFuncSetAttribute(k_xfft_prod<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
+    else CK(cudaFuncSetAttribute(k_xfft_prod<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
+    for (int j0 = 0; j0 < P.ny; j0 += h->pc) {
+        const int npl = (P.ny - j0 < h->pc) ? P.ny - j0 : h->pc;
+        int rc = zinv(h, Q, in, 6, j0, npl);
+        if (rc) return rc;
+        dim3 g(P.mz, npl);
+        PB(nprod == 3 ? CHAN_KC_XFFT_PROD : CHAN_KC_XFFT_PROD_FILTER);
+        if (nprod == 3) k_xfft_prod<3><<<g, 256, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
+        else k_xfft_prod<7><<<g, 256, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
+        LAUNCHED();
+        rc = zfwd(h, Q, pout, nprod, j0, npl, out, scale, nprod == 7, kxc, kzc);
+        if (rc) return rc;
+    }
+    return CHAN_OK;
+}
+
+int run_nonlinear(chan_t* h) {
+    FieldPtrsW out;
+    out.f[0] = h->H1; out.f[1] = h->H2; out.f[2] = h->H3;
+    return run_planes(h, 3, out, 0, 0);
+}
+
+// a9-a12
+int run_ysolve(chan_t* h) {
+    const Plan& P = h->P;
+    YParams Y = yparams(h);
+    MeanParams M;
+    M.ny = P.ny; M.nm = h->nm; M.A2 = h->tab[0][1]; M.B2 = h->tab[0][2]; M.wq = h->wq; M.wm = h->wm; M.wp = h->wp;
+    M.nu = P.nu; M.dt = P.dt; M.alpha = Y.alpha; M.beta = Y.beta; M.gamma = Y.gamma; M.zeta = Y.zeta; M.forcing = P.forcing;
+    PB(CHAN_KC_MEAN); k_mean<<<1, 32, 0, h->stream>>>(M, h->H1, h->H3, h->U, h->W, h->H1p, h->H3p, h->meanwork, h->scal); LAUNCHED();
+    const unsigned g = ygrid(h);
+    PB(CHAN_KC_Y1); k_y1<<<g, kThreadsY, 0, h->stream>>>(Y, h->H1, h->H3, h->omy, h->hg, h->z1, h->fac, h->z2); LAUNCHED();
+    PB(CHAN_KC_Y2); k_y2<<<g, kThreadsY, 0, h->stream>>>(Y, h->H2, h->z1, h->z2, h->fac, h->phi, h->hv, h->omy, h->z1, h->r1); LAUNCHED();
+    PB(CHAN_KC_Y3); k_y3<<<g, kThreadsY, 0, h->stream>>>(Y, h->fac, h->z1, h->r1, h->r2, h->z2, h->r3, h->r4); LAUNCHED();
+    PB(CHAN_KC_Y4); k_y4<<<g, kThreadsY, 0, h->stream>>>(Y, h->fac, h->z2, h->r3, h->r4, h->coef); LAUNCHED();
+    dim3 g5(g, P.ny < 64 ? P.ny : 64);
+    PB(CHAN_KC_Y5); k_y5<<<g5, kThreadsY, 0, h->stream>>>(Y, h->coef, h->z1, h->r2, h->r1, h->z2, h->r3, h->r4, h->phi, h->v); LAUNCHED();
+    return CHAN_OK;
+}
+
+int transpose(chan_t* h, int dir, const double2* in, double2* out) {
+    const long long nm = h->nm;
+    const int ny = h->P.ny;
+    const long long R = dir == 0 ? nm : ny, C = dir == 0 ? ny : nm;
+    dim3 g((unsigned)((C + 31) / 32), (unsigned)((R + 31) / 32));
+    PB(CHAN_KC_TRANSPOSE); k_transpose<<<g, 256, 0, h->stream>>>(in, out, nm, ny, dir); LAUNCHED();
+    return CHAN_OK;
+}
+
+double2* field_ptr(const chan_t* h, int f) {
+    switch (f) {
+        case CHAN_F_V: return h->v; case CHAN_F_PHI: return h->phi; case CHAN_F_OMY: return h->omy;
+        case CHAN_F_U: return h->u; case CHAN_F_W: return h->w; case CHAN_F_OMX: return h->ox; case CHAN_F_OMZ: return h->oz;
+        case CHAN_F_H1: return h->H1; case CHAN_F_H2: return h->H2; case CHAN_F_H3: return h->H3;
+        case CHAN_F_HV_PREV: return h->hv; case CHAN_F_HG_PREV: return h->hg;
+        default: return nullptr;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+int chan_create(chan_t** out, const chan_grid_t* grid, const chan_box_t* box, double re_tau, double dt, const chan_opts_t* opts) {
+    if (!out || !grid || !box) return CHAN_EINVAL;
+    *out = nullptr;
+    chan_t* h = new (std::nothrow) chan();
+    if (!h) return CHAN_ENOSPACE;
+    const int hl = opts ? opts->lhs_halfwidth : 3, hr = opts ? opts->rhs_halfwidth : 3, fo = opts ? opts->forcing : 0;
+    int rc = build_plan(h->P, grid->nx, grid->ny, grid->nz, box->lx, box->lz, box->y, re_tau, dt, hl ? hl : 3, hr ? hr : 3, fo);
+    if (rc != CHAN_OK) { delete h; return rc; }
+    if ((int)h->P.fx.radix.size() > CHAN_MAX_RADIX_PASSES || (int)h->P.fz.radix.size() > CHAN_MAX_RADIX_PASSES) { delete h; return CHAN_EINVAL; }
+    h->nm = (long long)h->P.nz * h->P.nxh;
+    h->F = (size_t)h->nm * h->P.ny * 16;
+    choose_tiling(h);
+    if ((size_t)3 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * 16 > 220 * 1024) { delete h; return CHAN_EINVAL; }
+    h->need = carve(h, nullptr);
+    *out = h;
+    return CHAN_OK;
+}
+
+int chan_destroy(chan_t* h) {
+    if (h) for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
+    delete h;
+    return CHAN_OK;
+}
+
+size_t chan_workspace_bytes(const chan_t* h) { return h ? h->need : 0; }
+
+int chan_bind(chan_t* h, void* dev_workspace, size_t bytes, void* cuda_stream) {
+    if (!h || !dev_workspace) return CHAN_EINVAL;
+    if (bytes < h->need) return CHAN_ENOSPACE;
+    if ((uintptr_t)dev_workspace % kAlign) return CHAN_EINVAL;
+    h->ws = (char*)dev_workspace; h->ws_bytes = bytes; h->stream = (cudaStream_t)cuda_stream;
+    carve(h, h->ws);
+    const Plan& P = h->P;
+    CK(cudaMemsetAsync(h->ws, 0, h->need, h->stream));
+    auto upl = [&](void* d, const void* s, size_t n) { return cudaMemcpyAsync(d, s, n, cudaMemcpyHostToDevice, h->stream); };
+    for (int o = 0; o < 2; ++o) {
+        CK(upl(h->tab[o][0], P.ot[o].B1.data(), P.ot[o].B1.size() * 8));
+        CK(upl(h->tab[o][1], P.ot[o].A2.data(), P.ot[o].A2.size() * 8));
+        CK(upl(h->tab[o][2], P.ot[o].B2.data(), P.ot[o].B2.size() * 8));
+        CK(upl(h->tab[o][3], P.ot[o].lu1.data(), P.ot[o].lu1.size() * 8));
+    }
+    CK(upl(h->kx, P.kx.data(), P.kx.size() * 8)); CK(upl(h->kz, P.kz.data(), P.kz.size() * 8));
+    CK(upl(h->wm, P.wm.data(), P.wm.size() * 8)); CK(upl(h->wp, P.wp.data(), P.wp.size() * 8));
+    CK(upl(h->wq, P.wq.data(), P.wq.size() * 8));
+    CK(upl(h->twx, P.fx.tw.data(), P.fx.tw.size() * 8)); CK(upl(h->twz, P.fz.tw.data(), P.fz.tw.size() * 8));
+    CK(cudaStreamSynchronize(h->stream));   // the host vectors may not outlive the copies otherwise
+    h->bound = true; h->have_state = false; h->isub = 0; h->nsamples = 0;
+    return CHAN_OK;
+}
+
+int chan_set_state(chan_t* h, const void* dv, const void* dphi, const void* domy, const double* dU, const double* dW) {
+    if (!h || !dv || !dphi || !domy || !dU || !dW) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    int rc;
+    if ((rc = transpose(h, 0, (const double2*)dv, h->v))) return rc;
+    if ((rc = transpose(h, 0, (const double2*)dphi, h->phi))) return rc;
+    if ((rc = transpose(h, 0, (const double2*)domy, h->omy))) return rc;
+    const Plan& P = h->P;
+    // the (0,0) mode and the z-Nyquist slot are not part of the state (reading R2)
+    for (double2* f : {h->v, h->phi, h->omy}) {
+        CK(cudaMemset2DAsync(f, (size_t)h->nm * 16, 0, 16, P.ny, h->stream));
+        CK(cudaMemset2DAsync(f + (size_t)P.nzh * P.nxh, (size_t)h->nm * 16, 0, (size_t)P.nxh * 16, P.ny, h->stream));
+    }
+    CK(cudaMemcpyAsync(h->U, dU, (size_t)P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->W, dW, (size_t)P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemsetAsync(h->hv, 0, h->F, h->stream)); CK(cudaMemsetAsync(h->hg, 0, h->F, h->stream));
+    CK(cudaMemsetAsync(h->H1p, 0, (size_t)P.ny * 8, h->stream)); CK(cudaMemsetAsync(h->H3p, 0, (size_t)P.ny * 8, h->stream));
+    PB(CHAN_KC_MEAN); k_flux<<<1, 32, 0, h->stream>>>(P.ny, h->wq, h->U, h->scal); LAUNCHED();
+    h->isub = 0; h->have_state = true;
+    return run_derive(h);
+}
+
+int chan_get_state(const chan_t* hc, void* dv, void* dphi, void* domy, double* dU, double* dW) {
+    chan_t* h = const_cast<chan_t*>(hc);
+    if (!h || !dv || !dphi || !domy || !dU || !dW) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    int rc;
+    if ((rc = transpose(h, 1, h->v, (double2*)dv))) return rc;
+    if ((rc = transpose(h, 1, h->phi, (double2*)dphi))) return rc;
+    if ((rc = transpose(h, 1, h->omy, (double2*)domy))) return rc;
+    CK(cudaMemcpyAsync(dU, h->U, (size_t)h->P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(dW, h->W, (size_t)h->P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
+    return CHAN_OK;
+}
+
+int chan_set_state_host(chan_t* h, const void* hv, const void* hphi, const void* homy, const double* hU, const double* hW) {
+    if (!h || !hv || !hphi || !homy || !hU || !hW) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    // stage the three fields in scratch (z1, z2, fac are idle between substeps), the profiles in meanwork
+    double2* st[3] = {h->z1, h->z2, (double2*)h->fac};
+    const void* src[3] = {hv, hphi, homy};
+    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(st[k], src[k], h->F, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->meanwork, hU, (size_t)h->P.ny * 8, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->meanwork + h->P.ny, hW, (size_t)h->P.ny * 8, cudaMemcpyHostToDevice, h->stream));
+    return chan_set_state(h, st[0], st[1], st[2], h->meanwork, h->meanwork + h->P.ny);
+}
+
+int chan_get_state_host(chan_t* h, void* hv, void* hphi, void* homy, double* hU, double* hW) {
+    if (!h || !hv || !hphi || !homy || !hU || !hW) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    double2* st[3] = {h->z1, h->z2, (double2*)h->fac};
+    int rc = chan_get_state(h, st[0], st[1], st[2], h->meanwork, h->meanwork + h->P.ny);
+    if (rc) return rc;
+    void* dst[3] = {hv, hphi, homy};
+    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], st[k], h->F, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaMemcpyAsync(hU, h->meanwork, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaMemcpyAsync(hW, h->meanwork + h->P.ny, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return CHAN_OK;
+}
+
+int chan_substep(chan_t* h) {
+    if (!h) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    int rc;
+    if ((rc = run_nonlinear(h))) return rc;
+    if ((rc = run_ysolve(h))) return rc;
+    h->isub = (h->isub + 1) % 3;
+    return run_derive(h);
+}
+
+int chan_step(chan_t* h) {
+    if (!h) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state || h->isub != 0) return CHAN_ESTATE;
+    for (int i = 0; i < 3; ++i) { int rc = chan_substep(h); if (rc) return rc; }
+    return CHAN_OK;
+}
+
+int chan_filter_store(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
+    if (!h || !dev_out) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
+    const size_t per = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1);
+    if (out_bytes < per * 10 * 16) return CHAN_ENOSPACE;
+    double2* out = (double2*)dev_out;
+    PlaneParams Q = pparams(h);
+    FieldPtrs in; in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w;
+    PB(CHAN_KC_FILTER_COPY); k_filter_copy<<<296, 256, 0, h->stream>>>(Q, in, out, kxc, kzc); LAUNCHED();
+    FieldPtrsW o;
+    for (int k = 0; k < 7; ++k) o.f[k] = out + (size_t)(3 + k) * per;
+    return run_planes(h, 7, o, kxc, kzc);
+}
+
+int chan_filter_store_host(chan_t* h, int kxc, int kzc, void* host_out, size_t out_bytes) {
+    if (!h || !host_out) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
+    const size_t bytes = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1) * 10 * 16;
+    if (out_bytes < bytes) return CHAN_ENOSPACE;
+    // staged in the y-phase scratch (fac, z1, z2, r1..r4 are contiguous: six fields), idle between substeps
+    if (bytes > (size_t)((char*)h->coef - (char*)h->fac)) return CHAN_ENOSPACE;
+    int rc = chan_filter_store(h, kxc, kzc, h->fac, bytes);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(host_out, h->fac, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return CHAN_OK;
+}
+
+int chan_stats(chan_t* h, int flags, double* host_out, long long* nsamples) {
+    if (!h) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if (flags & CHAN_STATS_RESET) {
+        CK(cudaMemsetAsync(h->stats, 0, (size_t)10 * P.ny * 8, h->stream));
+        h->nsamples = 0;
+    }
+    if (flags & CHAN_STATS_ACCUMULATE) {
+        if (!h->have_state) return CHAN_ESTATE;
+        PlaneParams Q = pparams(h);
+        FieldPtrs in; in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w; in.f[3] = h->ox; in.f[4] = h->omy; in.f[5] = h->oz;
+        PB(CHAN_KC_STATS); k_stats<<<P.ny, 256, 0, h->stream>>>(Q, in, h->stats); LAUNCHED();
+        ++h->nsamples;
+    }
+    if (flags & CHAN_STATS_READ) {
+        if (!host_out) return CHAN_EINVAL;
+        CK(cudaMemcpyAsync(host_out, h->stats, (size_t)10 * P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        if (nsamples) *nsamples = h->nsamples;
+    }
+    return CHAN_OK;
+}
+
+int chan_get_scalars(chan_t* h, double* out4) {
+    if (!h || !out4) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    CK(cudaMemcpyAsync(out4, h->scal, 32, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return CHAN_OK;
+}
+
+int chan_set_pgrad(chan_t* h, double g) {
+    if (!h) return CHAN_EINVAL;
+    if (!h->bound || h->P.forcing != 1) return CHAN_ESTATE;
+    CK(cudaMemcpyAsync(h->scal, &g, 8, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return CHAN_OK;
+}
+
+const char* chan_strerror(int s) {
+    switch (s) {
+        case CHAN_OK: return "ok";
+        case CHAN_EINVAL: return "invalid argument";
+        case CHAN_ENOSPACE: return "workspace or output buffer too small";
+        case CHAN_ESTATE: return "call out of order";
+        case CHAN_ECUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+int chan_debug_get_field(const chan_t* hc, int field, void* dev_out) {
+    chan_t* h = const_cast<chan_t*>(hc);
+    if (!h || !dev_out) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    double2* p = field_ptr(h, field);
+    if (!p) return CHAN_EINVAL;
+    return transpose(h, 1, p, (double2*)dev_out);
+}
+
+int chan_debug_set_field(chan_t* h, int field, const void* dev_in) {
+    if (!h || !dev_in) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    double2* p = field_ptr(h, field);
+    if (!p) return CHAN_EINVAL;
+    return transpose(h, 0, (const double2*)dev_in, p);
+}
+
+int chan_debug_run_stage(chan_t* h, int stage) {
+    if (!h) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    switch (stage) {
+        case CHAN_STAGE_DERIVE: return run_derive(h);
+        case CHAN_STAGE_NONLINEAR: return run_nonlinear(h);
+        case CHAN_STAGE_YSOLVE: return run_ysolve(h);
+        default: return CHAN_EINVAL;
+    }
+}
+
+int chan_debug_set_substep_index(chan_t* h, int i) {
+    if (!h || i < 0 || i > 2) return CHAN_EINVAL;
+    h->isub = i;
+    return CHAN_OK;
+}
+
+int chan_debug_get_band_tables(const chan_t* h, double* out) {
+    if (!h || !out) return CHAN_EINVAL;
+    const size_t n = (size_t)h->P.ny * 7;
+    std::memcpy(out, h->P.A1.data(), n * 8); std::memcpy(out + n, h->P.B1.data(), n * 8);
+    std::memcpy(out + 2 * n, h->P.A2.data(), n * 8); std::memcpy(out + 3 * n, h->P.B2.data(), n * 8);
+    return CHAN_OK;
+}
+
+long long chan_debug_launch_count(const chan_t* h) { return h ? h->launches : 0; }
+
+int chan_debug_profile(chan_t* h, int enable) {
+    if (!h) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    if (enable) {
+        for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
+        h->prof_ev.clear(); h->prof_cls.clear();
+    }
+    h->prof_on = enable != 0;
+    return CHAN_OK;
+}
+
+int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts) {
+    if (!h || !host_ms || !host_counts) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    CK(cudaStreamSynchronize(h->stream));
+    for (int k = 0; k < CHAN_KC_COUNT; ++k) { host_ms[k] = 0.0; host_counts[k] = 0; }
+    const size_t n = h->prof_cls.size();
+    for (size_t i = 0; i < n && 2 * i + 1 < h->prof_ev.size(); ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, h->prof_ev[2 * i], h->prof_ev[2 * i + 1]) == cudaSuccess) {
+            host_ms[h->prof_cls[i]] += ms; host_counts[h->prof_cls[i]] += 1;
+        }
+    }
+    return CHAN_OK;
+}
+
+int chan_debug_transpose(chan_t* h, int dir, const void* dev_in, void* dev_out) {
+    if (!h || !dev_in || !dev_out || dir < 0 || dir > 1) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    return transpose(h, dir, (const double2*)dev_in, (double2*)dev_out);
+}
+
+}  // extern "C"

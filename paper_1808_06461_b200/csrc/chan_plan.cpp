@@ -1,0 +1,283 @@
+// Host plan: compact finite-difference rows on the caller's mesh, their factorisations, wavenumbers,
+// FFT radix plans and twiddles.  long double throughout; rounded to double once.
+//
+// Compact rows ("seven-point compact finite differences", L100 "up to twelfth order of
+// consistency"; reading R4): row j of the d-th derivative satisfies
+//     sum_m a_m f^(d)(y_{j+m}) = sum_m b_m f(y_{j+m}),   a_0 = 1,
+// exactly for all polynomials up to degree (#unknowns - 1).  The moment system is written in the
+// Chebyshev basis T_k(t) on the stencil's own interval mapped to t in [-1,1] (reading R5), with the
+// b_m scaled by the half-width^d, and solved by partially pivoted elimination plus one refinement step.
+#include "chan_plan.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "../../include/chan.h"
+
+namespace chn {
+namespace {
+
+typedef long double ld;
+
+// Solve the dense n x n system M x = r (row-major M) by Gaussian elimination with partial pivoting.
+bool dense_solve(int n, std::vector<ld> M, std::vector<ld> r, std::vector<ld>& x) {
+    std::vector<int> perm(n);
+    for (int i = 0; i < n; ++i) perm[i] = i;
+    for (int c = 0; c < n; ++c) {
+        int p = c;
+        for (int i = c + 1; i < n; ++i)
+            if (fabsl(M[i * n + c]) > fabsl(M[p * n + c])) p = i;
+        if (M[p * n + c] == 0.0L) return false;
+        if (p != c) {
+            for (int k = 0; k < n; ++k) std::swap(M[c * n + k], M[p * n + k]);
+            std::swap(r[c], r[p]);
+        }
+        for (int i = c + 1; i < n; ++i) {
+            ld f = M[i * n + c] / M[c * n + c];
+            if (f == 0.0L) continue;
+            for (int k = c; k < n; ++k) M[i * n + k] -= f * M[c * n + k];
+            r[i] -= f * r[c];
+        }
+    }
+    x.assign(n, 0.0L);
+    for (int i = n - 1; i >= 0; --i) {
+        ld s = r[i];
+        for (int k = i + 1; k < n; ++k) s -= M[i * n + k] * x[k];
+        x[i] = s / M[i * n + i];
+    }
+    return true;
+}
+
+// T_k(t), T_k'(t), T_k''(t) for k = 0..n-1 by the three-term recurrences.
+void cheb_all(ld t, int n, std::vector<ld>& T0, std::vector<ld>& T1, std::vector<ld>& T2) {
+    T0.assign(n, 0); T1.assign(n, 0); T2.assign(n, 0);
+    T0[0] = 1;
+    if (n > 1) { T0[1] = t; T1[1] = 1; }
+    for (int k = 2; k < n; ++k) {
+        T0[k] = 2 * t * T0[k - 1] - T0[k - 2];
+        T1[k] = 2 * T0[k - 1] + 2 * t * T1[k - 1] - T1[k - 2];
+        T2[k] = 4 * T1[k - 1] + 2 * t * T2[k - 1] - T2[k - 2];
+    }
+}
+
+// One compact row.  lhs/rhs: offset lists (lhs contains 0).  Writes a[3+m], b[3+m].
+bool compact_row(const std::vector<double>& y, int j, const std::vector<int>& lhs, const std::vector<int>& rhs,
+                 int deriv, double* a, double* b) {
+    int lo = 0, hi = 0;
+    for (int m : lhs) { lo = std::min(lo, m); hi = std::max(hi, m); }
+    for (int m : rhs) { lo = std::min(lo, m); hi = std::max(hi, m); }
+    const ld ylo = y[j + lo], yhi = y[j + hi];
+    const ld ym = (ylo + yhi) / 2, hw = (yhi - ylo) / 2;
+    std::vector<int> lf;
+    for (int m : lhs) if (m != 0) lf.push_back(m);
+    const int n = (int)lf.size() + (int)rhs.size();
+    std::vector<ld> M((size_t)n * n), r(n), x, T0, T1, T2;
+    // column data per stencil point
+    auto fill = [&](int m, int col, bool is_lhs) {
+        ld t = ((ld)y[j + m] - ym) / hw;
+        cheb_all(t, n, T0, T1, T2);
+        for (int k = 0; k < n; ++k) {
+            ld v = is_lhs ? (deriv == 1 ? T1[k] : T2[k]) : -T0[k];
+            if (col >= 0) M[(size_t)k * n + col] = v; else r[k] = -v;  // col < 0: the a_0 = 1 term
+        }
+    };
+    int col = 0;
+    for (int m : lf) fill(m, col++, true);
+    for (int m : rhs) fill(m, col++, false);
+    fill(0, -1, true);
+    if (!dense_solve(n, M, r, x)) return false;
+    // one step of iterative refinement in the same precision (residual is cheap and exact enough)
+    std::vector<ld> res(n), dx;
+    for (int k = 0; k < n; ++k) {
+        ld s = r[k];
+        for (int c = 0; c < n; ++c) s -= M[(size_t)k * n + c] * x[c];
+        res[k] = s;
+    }
+    if (dense_solve(n, M, res, dx)) for (int k = 0; k < n; ++k) x[k] += dx[k];
+    for (int k = 0; k < 7; ++k) { a[k] = 0; b[k] = 0; }
+    a[3] = 1.0;
+    col = 0;
+    const ld sc = (deriv == 1) ? hw : hw * hw;  // unknown b' = b * hw^d  (LHS derivative columns carry 1/hw^d)
+    for (int m : lf) a[3 + m] = (double)x[col++];
+    for (int m : rhs) b[3 + m] = (double)(x[col++] / sc);
+    return true;
+}
+
+// Unpivoted band LU of a [ny][7] table in long double; writes rows {l1,l2,l3,1/u_ii,u1,u2,u3,0}.
+bool band_lu(int ny, const std::vector<ld>& T, std::vector<double>& out) {
+    std::vector<ld> W(T);
+    out.assign((size_t)ny * 8, 0.0);
+    std::vector<ld> L((size_t)ny * 3, 0.0L);
+    for (int j = 0; j < ny; ++j) {
+        ld piv = W[(size_t)j * 7 + 3];
+        if (piv == 0.0L) return false;
+        for (int t = 1; t <= 3 && j + t < ny; ++t) {
+            ld l = W[(size_t)(j + t) * 7 + 3 - t] / piv;
+            L[(size_t)(j + t) * 3 + (t - 1)] = l;
+            for (int cc = 1; cc <= 3; ++cc) W[(size_t)(j + t) * 7 + 3 - t + cc] -= l * W[(size_t)j * 7 + 3 + cc];
+            W[(size_t)(j + t) * 7 + 3 - t] = 0;
+        }
+    }
+    for (int j = 0; j < ny; ++j) {
+        double* o = &out[(size_t)j * 8];
+        o[0] = (double)L[(size_t)j * 3 + 0];
+        o[1] = (double)L[(size_t)j * 3 + 1];
+        o[2] = (double)L[(size_t)j * 3 + 2];
+        o[3] = (double)(1.0L / W[(size_t)j * 7 + 3]);
+        o[4] = (double)W[(size_t)j * 7 + 4];
+        o[5] = (double)W[(size_t)j * 7 + 5];
+        o[6] = (double)W[(size_t)j * 7 + 6];
+    }
+    return true;
+}
+
+// Solve T x = r for a [ny][7] band table without pivoting (long double).
+bool band_solve(int ny, const std::vector<ld>& T, std::vector<ld>& x) {
+    std::vector<ld> W(T);
+    for (int j = 0; j < ny; ++j) {
+        ld piv = W[(size_t)j * 7 + 3];
+        if (piv == 0.0L) return false;
+        for (int t = 1; t <= 3 && j + t < ny; ++t) {
+            ld l = W[(size_t)(j + t) * 7 + 3 - t] / piv;
+            for (int cc = 1; cc <= 3; ++cc) W[(size_t)(j + t) * 7 + 3 - t + cc] -= l * W[(size_t)j * 7 + 3 + cc];
+            x[j + t] -= l * x[j];
+        }
+    }
+    for (int j = ny - 1; j >= 0; --j) {
+        ld s = x[j];
+        for (int cc = 1; cc <= 3 && j + cc < ny; ++cc) s -= W[(size_t)j * 7 + 3 + cc] * x[j + cc];
+        x[j] = s / W[(size_t)j * 7 + 3];
+    }
+    return true;
+}
+
+void flip_table(int ny, const std::vector<double>& T, std::vector<double>& F) {  // F[i][3+m] = T[ny-1-i][3-m]
+    F.assign((size_t)ny * 7, 0.0);
+    for (int i = 0; i < ny; ++i)
+        for (int m = -3; m <= 3; ++m) F[(size_t)i * 7 + 3 + m] = T[(size_t)(ny - 1 - i) * 7 + 3 - m];
+}
+
+void pad8(int ny, const std::vector<double>& T, std::vector<double>& O) {
+    O.assign((size_t)ny * 8, 0.0);
+    for (int i = 0; i < ny; ++i) for (int k = 0; k < 7; ++k) O[(size_t)i * 8 + k] = T[(size_t)i * 7 + k];
+}
+
+bool make_fft_plan(int n, FftPlan& F) {
+    F.n = n;
+    F.radix.clear();
+    int r = n;
+    std::vector<int> twos, threes;
+    while (r % 3 == 0) { threes.push_back(3); r /= 3; }
+    int p2 = 0;
+    while (r % 2 == 0) { ++p2; r /= 2; }
+    if (r != 1 || n < 2) return false;
+    for (; p2 >= 2; p2 -= 2) F.radix.push_back(4);
+    if (p2) F.radix.push_back(2);
+    for (int t : threes) F.radix.push_back(t);
+    F.tw.resize((size_t)2 * n);
+    const ld two_pi = 6.283185307179586476925286766559005768L;
+    for (int k = 0; k < n; ++k) {
+        // exact octant reduction keeps the table symmetric to the last bit
+        ld a = two_pi * (ld)k / (ld)n;
+        F.tw[2 * k] = (double)cosl(a);
+        F.tw[2 * k + 1] = (double)(-sinl(a));
+    }
+    return true;
+}
+
+}  // namespace
+
+int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const double* y, double re_tau, double dt,
+               int half_lhs, int half_rhs, int forcing) {
+    if (nx < 4 || nz < 4 || (nx & 1) || (nz & 1) || ny < 8 || !y) return CHAN_EINVAL;
+    if (!(lx > 0) || !(lz > 0) || !(re_tau > 0) || !(dt > 0)) return CHAN_EINVAL;
+    if (half_lhs < 1 || half_lhs > 3 || half_rhs < 1 || half_rhs > 3 || forcing < 0 || forcing > 1) return CHAN_EINVAL;
+    for (int j = 1; j < ny; ++j) if (!(y[j] > y[j - 1])) return CHAN_EINVAL;
+    if (y[0] != -1.0 || y[ny - 1] != 1.0) return CHAN_EINVAL;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.nxh = nx / 2; P.nzh = nz / 2; P.mx = 3 * nx / 2; P.mz = 3 * nz / 2;
+    P.lx = lx; P.lz = lz; P.nu = 1.0 / re_tau; P.dt = dt;
+    P.half_lhs = half_lhs; P.half_rhs = half_rhs; P.forcing = forcing;
+    P.y.assign(y, y + ny);
+    if (!make_fft_plan(P.mx, P.fx) || !make_fft_plan(P.mz, P.fz)) return CHAN_EINVAL;
+
+    // RK3 constants of [34] (reading R3)
+    const double al[3] = {29.0 / 96.0, -3.0 / 40.0, 1.0 / 6.0}, be[3] = {37.0 / 160.0, 5.0 / 24.0, 1.0 / 6.0};
+    const double ga[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0}, ze[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
+    for (int i = 0; i < 3; ++i) { P.rk_alpha[i] = al[i]; P.rk_beta[i] = be[i]; P.rk_gamma[i] = ga[i]; P.rk_zeta[i] = ze[i]; }
+
+    // compact rows
+    P.A1.assign((size_t)ny * 7, 0.0); P.B1.assign((size_t)ny * 7, 0.0);
+    P.A2.assign((size_t)ny * 7, 0.0); P.B2.assign((size_t)ny * 7, 0.0);
+    for (int j = 0; j < ny; ++j) {
+        const int room = std::min(j, ny - 1 - j);
+        for (int d = 1; d <= 2; ++d) {
+            std::vector<int> lo, ro;
+            if (room == 0) {
+                if (d == 2) continue;
+                const int sg = (j == 0) ? 1 : -1;
+                lo = {0, sg};
+                ro = {0, sg, 2 * sg, 3 * sg};
+            } else {
+                const int sl = std::min(half_lhs, room), sr = std::min(half_rhs, room);
+                for (int m = -sl; m <= sl; ++m) lo.push_back(m);
+                for (int m = -sr; m <= sr; ++m) ro.push_back(m);
+            }
+            double* a = (d == 1 ? &P.A1[(size_t)j * 7] : &P.A2[(size_t)j * 7]);
+            double* b = (d == 1 ? &P.B1[(size_t)j * 7] : &P.B2[(size_t)j * 7]);
+            if (!compact_row(P.y, j, lo, ro, d, a, b)) return CHAN_EINVAL;
+        }
+    }
+
+    // orientation tables and the LU of A1 in both orientations
+    for (int o = 0; o < 2; ++o) {
+        std::vector<double> a1, b1, a2, b2;
+        if (o == 0) { a1 = P.A1; b1 = P.B1; a2 = P.A2; b2 = P.B2; }
+        else { flip_table(ny, P.A1, a1); flip_table(ny, P.B1, b1); flip_table(ny, P.A2, a2); flip_table(ny, P.B2, b2); }
+        pad8(ny, b1, P.ot[o].B1); pad8(ny, a2, P.ot[o].A2); pad8(ny, b2, P.ot[o].B2);
+        std::vector<ld> T(a1.begin(), a1.end());
+        if (!band_lu(ny, T, P.ot[o].lu1)) return CHAN_EINVAL;
+    }
+
+    // wall functionals: (D1 f)(wall) = e^T A1^{-1} B1 f = (A1^{-T} e)^T B1 f
+    {
+        std::vector<ld> At((size_t)ny * 7, 0.0L);
+        for (int j = 0; j < ny; ++j)
+            for (int m = -3; m <= 3; ++m)
+                if (j + m >= 0 && j + m < ny) At[(size_t)j * 7 + 3 + m] = P.A1[(size_t)(j + m) * 7 + 3 - m];
+        for (int side = 0; side < 2; ++side) {
+            std::vector<ld> s(ny, 0.0L);
+            s[side == 0 ? 0 : ny - 1] = 1.0L;
+            if (!band_solve(ny, At, s)) return CHAN_EINVAL;
+            std::vector<double>& w = (side == 0 ? P.wm : P.wp);
+            w.assign(ny, 0.0);
+            for (int c = 0; c < ny; ++c) {
+                ld acc = 0;
+                for (int m = -3; m <= 3; ++m) {  // w_c = sum_j s_j B1[j][c], j = c - m
+                    int j = c - m;
+                    if (j >= 0 && j < ny) acc += s[j] * (ld)P.B1[(size_t)j * 7 + 3 + m];
+                }
+                w[c] = (double)acc;
+            }
+        }
+    }
+
+    // trapezoid weights (reading R8)
+    P.wq.assign(ny, 0.0);
+    for (int j = 0; j + 1 < ny; ++j) {
+        const double h = 0.5 * (P.y[j + 1] - P.y[j]);
+        P.wq[j] += h; P.wq[j + 1] += h;
+    }
+
+    // wavenumbers (reading R2)
+    const double two_pi = 6.283185307179586476925286766559;
+    P.kx.resize(P.nxh); P.kz.resize(nz);
+    for (int p = 0; p < P.nxh; ++p) P.kx[p] = two_pi * p / lx;
+    for (int s = 0; s < nz; ++s) {
+        int q = (s < P.nzh) ? s : (s == P.nzh ? 0 : s - nz);
+        P.kz[s] = two_pi * q / lz;
+    }
+    return CHAN_OK;
+}
+
+}  // namespace chn

