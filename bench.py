@@ -99,7 +99,7 @@ def pick_workload(name, free_bytes):
     for cand in ("cfg5", "cfg4", "cfg3"):
         c = inputs.CONFIGS[cand]
         F = c["nx"] * c["ny"] * c["nz"] * 8
-        if 15.6 * F + 4e9 < free_bytes:      # workspace (15 fields + chunks) + slack
+        if 10.3 * F + 8e9 < free_bytes:      # workspace (10 fields + plane chunks) + filter output + slack
             return cand
     return "mid"
 
@@ -186,16 +186,24 @@ def main():
     F = npts * 8
     kxc, kzc = c["cut"]
 
-    # ---- inputs resident in HBM ---------------------------------------------------------------------
-    v, phi, omy = inputs.fluctuations(c, device=dev)
-    U = torch.from_numpy(c["U"]).to(dev)
-    Wm = torch.from_numpy(c["W"]).to(dev)
+    # ---- inputs: built slab by slab on the device into pinned host buffers (they are also the e2e leg's host
+    # side), handed to the library once through chan_set_state_host, so that the state is resident in HBM
+    # inside the library's workspace before the timed region and no second device copy competes for memory
+    shape = (c["nz"], c["nx"] // 2, c["ny"])
+    try:
+        hv, hp, ho = (torch.empty(shape, dtype=torch.complex128, pin_memory=True) for _ in range(3))
+        pinned = True
+    except RuntimeError:
+        hv, hp, ho = (torch.empty(shape, dtype=torch.complex128) for _ in range(3))
+        pinned = False
+    inputs.fluctuations(c, device=dev, zchunk=max(1, min(c["nz"], (1 << 31) // (c["nx"] // 2 * c["ny"] * 16))), out=(hv, hp, ho))
+    hU = torch.from_numpy(c["U"]).clone()
+    hW = torch.from_numpy(c["W"]).clone()
     torch.cuda.empty_cache()
     ch = binding.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
     ws_bytes = ch.workspace_bytes()
     ch.bind(dev)
-    ch.set_state(v, phi, omy, U, Wm)
-    ch._keep = None
+    ch.set_state_host(hv, hp, ho, hU, hW)
     fout = torch.empty((10, c["ny"], 2 * kzc + 1, kxc + 1), dtype=torch.complex128, device=dev)
     stream = ch.stream
 
@@ -232,10 +240,9 @@ def main():
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
     ms_total_max = float(tmax.item())
     value = world * 3 * npts * K / (ms_total_max * 1e-3) / 1e6
-    # finite-state check: a blown-up field would make the timing meaningless
-    gv = ch.get_state()[0]
-    finite = bool(torch.isfinite(torch.view_as_real(gv)).all().item())
-    del gv
+    # finite-state check: a blown-up field would make the timing meaningless (the ten filtered variables
+    # are linear and quadratic in every velocity and vorticity component)
+    finite = bool(torch.isfinite(torch.view_as_real(fout)).all().item())
 
     # ---- substeps alone -----------------------------------------------------------------------------
     barrier()
@@ -287,12 +294,7 @@ def main():
     if rank == 0 or world > 1:
         Ke = max(1, min(args.e2e_steps, K))
         try:
-            hv = torch.empty(ch.shape, dtype=torch.complex128, pin_memory=True)
-            hp = torch.empty(ch.shape, dtype=torch.complex128, pin_memory=True)
-            ho = torch.empty(ch.shape, dtype=torch.complex128, pin_memory=True)
-            hU = torch.empty(c["ny"], dtype=torch.float64, pin_memory=True)
-            hW = torch.empty(c["ny"], dtype=torch.float64, pin_memory=True)
-            hf = torch.empty(tuple(fout.shape), dtype=torch.complex128, pin_memory=True)
+            hf = torch.empty(tuple(fout.shape), dtype=torch.complex128, pin_memory=pinned)
             ch.get_state_host(hv, hp, ho, hU, hW)
 
             def e2e_step():
@@ -319,8 +321,9 @@ def main():
             e2e = {"value": world * 3 * npts * Ke / (float(te.item()) * 1e-3) / 1e6, "unit": UNIT, "steps": Ke,
                    "ms_per_step": float(te.item()) / Ke, "h2d_bytes_per_step": state_b,
                    "d2h_bytes_per_step": state_b + hf.numel() * 16 + 10 * c["ny"] * 8,
-                   "api": "chan_set_state_host + chan_step + chan_filter_store_host + chan_stats(READ) + chan_get_state_host, pinned host buffers"}
-            del hv, hp, ho, hf
+                   "api": "chan_set_state_host + chan_step + chan_filter_store_host + chan_stats(READ) + chan_get_state_host, "
+                          + ("pinned" if pinned else "pageable (pinning refused)") + " host buffers"}
+            del hf
         except RuntimeError as ex:      # pinned allocation refused by the host
             e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
 

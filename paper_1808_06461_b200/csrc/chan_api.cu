@@ -32,13 +32,16 @@ struct chan {
     int cuda_err = 0;
     // sizes
     size_t F = 0;          // bytes of one complex field
+    size_t s1_bytes = 0;   // bytes of the scratch field s1 (>= F; also the host staging of the filter output)
     long long nm = 0;
     int pc = 1;            // planes per FFT chunk
     int Tz = 1;            // k_x columns per z-FFT tile
     // device pointers (carved)
     double2 *v, *phi, *omy, *hv, *hg, *u, *w, *ox, *oz;   // plane layout fields
     double2 *H1, *H2, *H3;                                 // alias u, w, ox
-    double4* fac; double2 *z1, *z2; double *r1, *r2, *r3, *r4; double4* coef;
+    // y-phase scratch: only s1 is storage of its own, the rest alias field buffers that are dead while the
+    // y-phase runs: facA = oz, facB = v, z2 = u, r1|r2 = ox, r3|r4 = w
+    double2 *s1, *facA, *facB, *z1, *z2; double *r1, *r2, *r3, *r4; double4* coef;
     double2 *zpad, *xh;
     double *U, *W, *H1p, *H3p, *meanwork, *scal, *stats;
     // tables
@@ -82,9 +85,12 @@ size_t carve(chan_t* h, char* base) {
     h->hv = c.take<double2>(F); h->hg = c.take<double2>(F);
     h->u = c.take<double2>(F); h->w = c.take<double2>(F); h->ox = c.take<double2>(F); h->oz = c.take<double2>(F);
     h->H1 = h->u; h->H2 = h->w; h->H3 = h->ox;
-    h->fac = c.take<double4>(2 * F);
-    h->z1 = c.take<double2>(F); h->z2 = c.take<double2>(F);
-    h->r1 = c.take<double>(F / 2); h->r2 = c.take<double>(F / 2); h->r3 = c.take<double>(F / 2); h->r4 = c.take<double>(F / 2);
+    h->s1_bytes = F > ((size_t)64 << 20) ? F : (10 * F < ((size_t)64 << 20) ? 10 * F : ((size_t)64 << 20));
+    h->s1 = c.take<double2>(h->s1_bytes);
+    h->z1 = h->s1; h->z2 = h->u; h->facA = h->oz; h->facB = h->v;
+    const size_t half = (size_t)h->nm * P.ny;     // doubles in half a field
+    h->r1 = (double*)h->ox; h->r2 = h->r1 ? h->r1 + half : nullptr;
+    h->r3 = (double*)h->w; h->r4 = h->r3 ? h->r3 + half : nullptr;
     h->coef = c.take<double4>((size_t)h->nm * 32);
     h->zpad = c.take<double2>((size_t)6 * h->pc * P.mz * P.nxh * 16);
     h->xh = c.take<double2>((size_t)7 * h->pc * P.mz * P.nxh * 16);
@@ -144,8 +150,8 @@ inline unsigned ygrid(const chan_t* h) { return (unsigned)((h->nm + kThreadsY - 
 int run_derive(chan_t* h) {
     YParams Y = yparams(h);
     PB(CHAN_KC_D1FWD); k_d1_forward<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->v, h->z1); LAUNCHED();
-    PB(CHAN_KC_DERIVE_DOWN); k_derive_down<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->z1, h->omy, h->U, h->W, h->u, h->w, h->z2, (double2*)h->fac); LAUNCHED();
-    PB(CHAN_KC_DERIVE_UP); k_derive_up<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->z2, (double2*)h->fac, h->v, h->ox, h->oz); LAUNCHED();
+    PB(CHAN_KC_DERIVE_DOWN); k_derive_down<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->z1, h->omy, h->U, h->W, h->u, h->w, h->s1, h->oz); LAUNCHED();
+    PB(CHAN_KC_DERIVE_UP); k_derive_up<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->s1, h->oz, h->v, h->ox, h->oz); LAUNCHED();
     return CHAN_OK;
 }
 
@@ -224,10 +230,10 @@ int run_ysolve(chan_t* h) {
     M.nu = P.nu; M.dt = P.dt; M.alpha = Y.alpha; M.beta = Y.beta; M.gamma = Y.gamma; M.zeta = Y.zeta; M.forcing = P.forcing;
     PB(CHAN_KC_MEAN); k_mean<<<1, 32, 0, h->stream>>>(M, h->H1, h->H3, h->U, h->W, h->H1p, h->H3p, h->meanwork, h->scal); LAUNCHED();
     const unsigned g = ygrid(h);
-    PB(CHAN_KC_Y1); k_y1<<<g, kThreadsY, 0, h->stream>>>(Y, h->H1, h->H3, h->omy, h->hg, h->z1, h->fac, h->z2); LAUNCHED();
-    PB(CHAN_KC_Y2); k_y2<<<g, kThreadsY, 0, h->stream>>>(Y, h->H2, h->z1, h->z2, h->fac, h->phi, h->hv, h->omy, h->z1, h->r1); LAUNCHED();
-    PB(CHAN_KC_Y3); k_y3<<<g, kThreadsY, 0, h->stream>>>(Y, h->fac, h->z1, h->r1, h->r2, h->z2, h->r3, h->r4); LAUNCHED();
-    PB(CHAN_KC_Y4); k_y4<<<g, kThreadsY, 0, h->stream>>>(Y, h->fac, h->z2, h->r3, h->r4, h->coef); LAUNCHED();
+    PB(CHAN_KC_Y1); k_y1<<<g, kThreadsY, 0, h->stream>>>(Y, h->H1, h->H3, h->omy, h->hg, h->z1, h->facA, h->facB, h->z2); LAUNCHED();
+    PB(CHAN_KC_Y2); k_y2<<<g, kThreadsY, 0, h->stream>>>(Y, h->H2, h->z1, h->z2, h->facA, h->facB, h->phi, h->hv, h->omy, h->z1, h->r1); LAUNCHED();
+    PB(CHAN_KC_Y3); k_y3<<<g, kThreadsY, 0, h->stream>>>(Y, h->facA, h->facB, h->z1, h->r1, h->r2, h->z2, h->r3, h->r4); LAUNCHED();
+    PB(CHAN_KC_Y4); k_y4<<<g, kThreadsY, 0, h->stream>>>(Y, h->facA, h->facB, h->z2, h->r3, h->r4, h->coef); LAUNCHED();
     dim3 g5(g, P.ny < 64 ? P.ny : 64);
     PB(CHAN_KC_Y5); k_y5<<<g5, kThreadsY, 0, h->stream>>>(Y, h->coef, h->z1, h->r2, h->r1, h->z2, h->r3, h->r4, h->phi, h->v); LAUNCHED();
     return CHAN_OK;
@@ -344,8 +350,8 @@ int chan_get_state(const chan_t* hc, void* dv, void* dphi, void* domy, double* d
 int chan_set_state_host(chan_t* h, const void* hv, const void* hphi, const void* homy, const double* hU, const double* hW) {
     if (!h || !hv || !hphi || !homy || !hU || !hW) return CHAN_EINVAL;
     if (!h->bound) return CHAN_ESTATE;
-    // stage the three fields in scratch (z1, z2, fac are idle between substeps), the profiles in meanwork
-    double2* st[3] = {h->z1, h->z2, (double2*)h->fac};
+    // stage the three fields in the derived-field buffers (rebuilt by set_state), the profiles in meanwork
+    double2* st[3] = {h->u, h->w, h->ox};
     const void* src[3] = {hv, hphi, homy};
     for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(st[k], src[k], h->F, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyAsync(h->meanwork, hU, (size_t)h->P.ny * 8, cudaMemcpyHostToDevice, h->stream));
@@ -356,13 +362,15 @@ int chan_set_state_host(chan_t* h, const void* hv, const void* hphi, const void*
 int chan_get_state_host(chan_t* h, void* hv, void* hphi, void* homy, double* hU, double* hW) {
     if (!h || !hv || !hphi || !homy || !hU || !hW) return CHAN_EINVAL;
     if (!h->bound || !h->have_state) return CHAN_ESTATE;
-    double2* st[3] = {h->z1, h->z2, (double2*)h->fac};
+    // staged in the derived-field buffers u, w, om_x, which are rebuilt (step a1) after the copies are queued
+    double2* st[3] = {h->u, h->w, h->ox};
     int rc = chan_get_state(h, st[0], st[1], st[2], h->meanwork, h->meanwork + h->P.ny);
     if (rc) return rc;
     void* dst[3] = {hv, hphi, homy};
     for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], st[k], h->F, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaMemcpyAsync(hU, h->meanwork, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaMemcpyAsync(hW, h->meanwork + h->P.ny, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
+    if ((rc = run_derive(h))) return rc;
     CK(cudaStreamSynchronize(h->stream));
     return CHAN_OK;
 }
@@ -407,11 +415,11 @@ int chan_filter_store_host(chan_t* h, int kxc, int kzc, void* host_out, size_t o
     if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
     const size_t bytes = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1) * 10 * 16;
     if (out_bytes < bytes) return CHAN_ENOSPACE;
-    // staged in the y-phase scratch (fac, z1, z2, r1..r4 are contiguous: six fields), idle between substeps
-    if (bytes > (size_t)((char*)h->coef - (char*)h->fac)) return CHAN_ENOSPACE;
-    int rc = chan_filter_store(h, kxc, kzc, h->fac, bytes);
+    // staged in the y-phase scratch field s1 (idle between substeps): at most one field's worth of output
+    if (bytes > h->s1_bytes) return CHAN_ENOSPACE;
+    int rc = chan_filter_store(h, kxc, kzc, h->s1, bytes);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(host_out, h->fac, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaMemcpyAsync(host_out, h->s1, bytes, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return CHAN_OK;
 }

@@ -128,6 +128,15 @@ template <> __device__ __forceinline__ double RhsFwd<double>::step(const HeptaFa
     z3 = z2; z2 = z1; z1 = z;
     return z;
 }
+// A factor row {1/d, u1, u2, u3} is stored as two double2 halves in two separate arrays (facA = {1/d, u1},
+// facB = {u2, u3}) so that each half can live in a different dead field buffer.
+__device__ __forceinline__ void st_fac(double2* fa, double2* fb, size_t o, double4 f) {
+    fa[o] = make_double2(f.x, f.y); fb[o] = make_double2(f.z, f.w);
+}
+__device__ __forceinline__ double4 ld_fac(const double2* fa, const double2* fb, size_t o) {
+    const double2 a = fa[o], b = fb[o];
+    return make_double4(a.x, a.y, b.x, b.y);
+}
 template <typename T> struct RhsBwd {   // back substitution with a stored factor row
     T x1, x2, x3;
     __device__ __forceinline__ T step(double4 f, T z);
@@ -180,14 +189,17 @@ __global__ void __launch_bounds__(128) k_d1_forward(YParams P, const double2* __
 // K1b (physical rows descending): dv = backsub(zv); u,w from (dv, om_y) [mode 0: U,W]; store u,w;
 // forward-eliminate (orientation 1) B1 u and B1 w -> zu, zw.
 // =====================================================================================================
-__global__ void __launch_bounds__(128) k_derive_down(YParams P, const double2* __restrict__ zv, const double2* __restrict__ omy,
+__global__ void __launch_bounds__(128) k_derive_down(YParams P, const double2* zv, const double2* __restrict__ omy,
                                                      const double* __restrict__ U, const double* __restrict__ W,
                                                      double2* __restrict__ u, double2* __restrict__ w_,
-                                                     double2* __restrict__ zu, double2* __restrict__ zw) {
+                                                     double2* zu /* may alias zv */, double2* __restrict__ zw) {
     long long m; int s, p; double kx, kz;
     if (!mode_setup(P, m, s, p, kx, kz)) return;
-    if (s == P.nzh) return;
     const int ny = P.ny;
+    if (s == P.nzh) {   // z-Nyquist slot: always zero (the buffers double as y-phase scratch)
+        for (int j = 0; j < ny; ++j) { stc(u + (size_t)j * P.nm + m, mk(0, 0)); stc(w_ + (size_t)j * P.nm + m, mk(0, 0)); }
+        return;
+    }
     const bool mean = (m == 0);
     const double k2 = kx * kx + kz * kz;
     const double ik2 = mean ? 0.0 : 1.0 / k2;
@@ -231,12 +243,15 @@ __global__ void __launch_bounds__(128) k_derive_down(YParams P, const double2* _
 // K1c (physical rows ascending): du, dw = backsub (orientation 1) of zu, zw;
 // om_x = dw - i kz v, om_z = i kx v - du.
 // =====================================================================================================
-__global__ void __launch_bounds__(128) k_derive_up(YParams P, const double2* __restrict__ zu, const double2* __restrict__ zw,
-                                                   const double2* __restrict__ v, double2* __restrict__ ox, double2* __restrict__ oz) {
+__global__ void __launch_bounds__(128) k_derive_up(YParams P, const double2* __restrict__ zu, const double2* zw /* may alias oz */,
+                                                   const double2* __restrict__ v, double2* __restrict__ ox, double2* oz) {
     long long m; int s, p; double kx, kz;
     if (!mode_setup(P, m, s, p, kx, kz)) return;
-    if (s == P.nzh) return;
     const int ny = P.ny;
+    if (s == P.nzh) {
+        for (int j = 0; j < ny; ++j) { stc(ox + (size_t)j * P.nm + m, mk(0, 0)); stc(oz + (size_t)j * P.nm + m, mk(0, 0)); }
+        return;
+    }
     D1Bwd bu, bw; bu.init(); bw.init();
     double luf[8];
     for (int j = 0; j < ny; ++j) {
@@ -279,9 +294,9 @@ __device__ __forceinline__ c2 helm_rhs(const YParams& P, int i, double c, double
 //   zd  = D1-forward(orientation 0) of d,
 //   om_y Helmholtz (B2 - lam A2) x = R_om, forward elimination in orientation 0 -> fac, z_om.
 // =====================================================================================================
-__global__ void __launch_bounds__(128) k_y1(YParams P, const double2* __restrict__ H1, const double2* __restrict__ H3,
+__global__ void __launch_bounds__(128) k_y1(YParams P, const double2* H1, const double2* __restrict__ H3,
                                             const double2* __restrict__ omy, double2* __restrict__ hg,
-                                            double2* __restrict__ zd, double4* __restrict__ fac, double2* __restrict__ zom) {
+                                            double2* __restrict__ zd, double2* __restrict__ facA, double2* __restrict__ facB, double2* zom) {
     long long m; int s, p; double kx, kz;
     if (!mode_setup(P, m, s, p, kx, kz)) return;
     if (s == P.nzh || m == 0) return;
@@ -315,7 +330,7 @@ __global__ void __launch_bounds__(128) k_y1(YParams P, const double2* __restrict
             load8(P.t[0].A2, j, a2); load8(P.t[0].B2, j, b2);
             helm_row(P, 0, j, lam, a2, b2, a);
             c2 r = helm_rhs(P, j, c, k2, a2, b2, wt, wx);
-            fac[o] = hf.reduce(a);
+            st_fac(facA, facB, o, hf.reduce(a));
             stc(zom + o, rz.step(hf, r));
         }
     }
@@ -327,7 +342,7 @@ __global__ void __launch_bounds__(128) k_y1(YParams P, const double2* __restrict
 //   (z of the homogeneous problem with phi(+1)=1; the one with phi(-1)=1 has z = unit vector, not stored).
 // =====================================================================================================
 __global__ void __launch_bounds__(128) k_y2(YParams P, const double2* __restrict__ H2, const double2* zd,
-                                            const double2* __restrict__ zom, double4* __restrict__ fac,
+                                            const double2* __restrict__ zom, double2* facA, double2* facB,
                                             const double2* __restrict__ phi, double2* __restrict__ hv, double2* __restrict__ omy,
                                             double2* zphi, double* __restrict__ zb) {
     long long m; int s, p; double kx, kz;
@@ -349,7 +364,7 @@ __global__ void __launch_bounds__(128) k_y2(YParams P, const double2* __restrict
         const int j = ny - 1 - ii;
         if (ii < ny) {
             const size_t o = (size_t)j * P.nm + m;
-            stc(omy + o, bo.step(fac[o], ldc(zom + o)));
+            stc(omy + o, bo.step(ld_fac(facA, facB, o), ldc(zom + o)));
             load8(P.t[0].lu1, j, lu);
             c2 dd = bd.step(lu, ldc(zd + o));
             c2 h2 = ldc(H2 + o), x = ldc(phi + o), hp = ldc(hv + o);
@@ -364,7 +379,7 @@ __global__ void __launch_bounds__(128) k_y2(YParams P, const double2* __restrict
             load8(P.t[1].A2, i, a2); load8(P.t[1].B2, i, b2);
             helm_row(P, 1, i, lam, a2, b2, a);
             c2 r = helm_rhs(P, i, c, k2, a2, b2, wt, wx);
-            fac[o] = hf.reduce(a);
+            st_fac(facA, facB, o, hf.reduce(a));
             stc(zphi + o, rz.step(hf, r));
             zb[o] = rb.step(hf, i == 0 ? 1.0 : 0.0);   // virtual row 0 = physical wall y=+1
         }
@@ -375,7 +390,7 @@ __global__ void __launch_bounds__(128) k_y2(YParams P, const double2* __restrict
 // Y3 (ascending): phi_p, phi_a, phi_b = backsub (orientation 1);  Poisson (B2 - k2 A2) v_s = A2 phi_s,
 //   forward elimination in orientation 0 -> fac (overwritten), z_vp, z_va, z_vb.
 // =====================================================================================================
-__global__ void __launch_bounds__(128) k_y3(YParams P, double4* __restrict__ fac, double2* __restrict__ zphi /* -> phi_p */,
+__global__ void __launch_bounds__(128) k_y3(YParams P, double2* facA, double2* facB, double2* __restrict__ zphi /* -> phi_p */,
                                             double* __restrict__ zb /* -> phi_b */, double* __restrict__ phia,
                                             double2* __restrict__ zvp, double* __restrict__ zva, double* __restrict__ zvb) {
     long long m; int s, p; double kx, kz;
@@ -395,7 +410,7 @@ __global__ void __launch_bounds__(128) k_y3(YParams P, double4* __restrict__ fac
     for (int jj = 0; jj < ny + 3; ++jj) {
         if (jj < ny) {
             const size_t o = (size_t)jj * P.nm + m;
-            const double4 f = fac[o];
+            const double4 f = ld_fac(facA, facB, o);
             c2 pp = bp.step(f, ldc(zphi + o));
             double pb = bb.step(f, zb[o]);
             double pa = ba.step(f, jj == 0 ? 1.0 : 0.0);   // z of the phi(-1)=1 problem: unit vector at the last virtual row
@@ -410,7 +425,7 @@ __global__ void __launch_bounds__(128) k_y3(YParams P, double4* __restrict__ fac
             const bool wall = (j == 0 || j == ny - 1);
             c2 r = wall ? mk(0, 0) : band7(a2, wp_);
             double rra = wall ? 0.0 : band7(a2, wa), rrb = wall ? 0.0 : band7(a2, wb);
-            fac[o] = hf.reduce(a);
+            st_fac(facA, facB, o, hf.reduce(a));
             stc(zvp + o, rp.step(hf, r));
             zva[o] = ra.step(hf, rra);
             zvb[o] = rb.step(hf, rrb);
@@ -422,7 +437,7 @@ __global__ void __launch_bounds__(128) k_y3(YParams P, double4* __restrict__ fac
 // Y4 (descending): v_p, v_a, v_b = backsub (orientation 0); wall derivatives as weighted sums;
 //   influence matrix (step 7) -> coef[m] = (c_a, c_b).
 // =====================================================================================================
-__global__ void __launch_bounds__(128) k_y4(YParams P, const double4* __restrict__ fac, double2* __restrict__ zvp,
+__global__ void __launch_bounds__(128) k_y4(YParams P, const double2* __restrict__ facA, const double2* __restrict__ facB, double2* __restrict__ zvp,
                                             double* __restrict__ zva, double* __restrict__ zvb, double4* __restrict__ coef) {
     long long m; int s, p; double kx, kz;
     if (!mode_setup(P, m, s, p, kx, kz)) return;
@@ -434,7 +449,7 @@ __global__ void __launch_bounds__(128) k_y4(YParams P, const double4* __restrict
     double dam = 0, dap = 0, dbm = 0, dbp = 0;
     for (int j = ny - 1; j >= 0; --j) {
         const size_t o = (size_t)j * P.nm + m;
-        const double4 f = fac[o];
+        const double4 f = ld_fac(facA, facB, o);
         c2 vp = bp.step(f, ldc(zvp + o));
         double va = ba.step(f, zva[o]), vb = bb.step(f, zvb[o]);
         stc(zvp + o, vp); zva[o] = va; zvb[o] = vb;

@@ -107,12 +107,15 @@ def _amplitude(k2, spec):
     return torch.sqrt(e / torch.clamp(kh, min=1e-30))
 
 
-def fluctuations(c, device="cpu", layout="line"):
+def fluctuations(c, device="cpu", layout="line", zchunk=None, out=None):
     """Seeded (v^, phi^, om_y^) for config dict ``c``; complex128 torch tensors on ``device``.
 
     layout "line": [nz][nx/2][ny] (the C ABI's state layout).  The rescale uses only analytic
     quantities (u^, w^ from the polynomial dv/dy): "maxu" = max over the nx x nz collocation grid of
     |u - <u>|, "rms" = plane- and y-point-averaged (u'^2+v'^2+w'^2)/3 = amp^2.
+    ``zchunk``: build the fields in slabs of that many k_z slots (bounds the temporaries for the large
+    configs; "rms" rescale only).  ``out``: optional triple of preallocated [nz][nx/2][ny] complex128
+    tensors (any device, e.g. pinned host memory) that receive the result slab by slab.
     """
     nx, ny, nz, M = c["nx"], c["ny"], c["nz"], c["M"]
     nxh, nzh = nx // 2, nz // 2
@@ -135,30 +138,49 @@ def fluctuations(c, device="cpu", layout="line"):
     P, Q = _basis_tables(c["y"], M)
     P = torch.from_numpy(P).to(dev).to(torch.complex128)
     Q = torch.from_numpy(Q).to(dev).to(torch.complex128)
-    cv = coef[0] * amp[:, :, None]
-    cw = coef[1] * amp[:, :, None]
-    v = cv @ P[0]
-    dv = cv @ P[1]
-    phi = cv @ P[2] - k2[:, :, None] * v
-    omy = cw @ Q
-    # analytic u^, w^ for the rescale
     k2s = k2.clone()
     k2s[0, 0] = 1.0
     k2s[nzh, :] = 1.0
-    u = 1j * (kx[None, :, None] * dv - kz[:, None, None] * omy) / k2s[:, :, None]
-    w = 1j * (kz[:, None, None] * dv + kx[None, :, None] * omy) / k2s[:, :, None]
     kind, target = c["amp"]
-    if kind == "maxu":
-        full = torch.zeros((nz, nxh + 1, ny), dtype=torch.complex128, device=dev)
-        full[:, :nxh] = u
-        phys = torch.fft.irfft(torch.fft.ifft(full, dim=0) * nz, n=nx, dim=1) * nx
-        scale = target / float(phys.abs().max())
-    else:
-        wp = torch.full((nxh,), 2.0, dtype=torch.float64, device=dev)
-        wp[0] = 1.0
-        e = ((u.abs() ** 2 + v.abs() ** 2 + w.abs() ** 2) * wp[None, :, None]).sum() / (3.0 * ny)
-        scale = target / math.sqrt(float(e))
-    v, phi, omy = v * scale, phi * scale, omy * scale
+    step = nz if (zchunk is None or kind == "maxu") else int(zchunk)
+    if out is None:
+        out = tuple(torch.empty((nz, nxh, ny), dtype=torch.complex128, device=dev) for _ in range(3))
+    wp = torch.full((nxh,), 2.0, dtype=torch.float64, device=dev)
+    wp[0] = 1.0
+    def slab(sl):
+        cv = coef[0, sl] * amp[sl, :, None]
+        cw = coef[1, sl] * amp[sl, :, None]
+        v = cv @ P[0]
+        dv = cv @ P[1]
+        phi = cv @ P[2] - k2[sl, :, None] * v
+        omy = cw @ Q
+        return v, dv, phi, omy
+
+    slabs = [slice(z0, min(nz, z0 + step)) for z0 in range(0, nz, step)]
+    esum, umax, keep = 0.0, 0.0, None
+    for sl in slabs:  # pass 1: the norm used by the rescale (analytic u^, w^)
+        v, dv, phi, omy = slab(sl)
+        u = 1j * (kx[None, :, None] * dv - kz[sl, None, None] * omy) / k2s[sl, :, None]
+        w = 1j * (kz[sl, None, None] * dv + kx[None, :, None] * omy) / k2s[sl, :, None]
+        del dv
+        if kind == "maxu":
+            full = torch.zeros((nz, nxh + 1, ny), dtype=torch.complex128, device=dev)
+            full[:, :nxh] = u
+            phys = torch.fft.irfft(torch.fft.ifft(full, dim=0) * nz, n=nx, dim=1) * nx
+            umax = float(phys.abs().max())
+        else:
+            esum += float(((u.abs() ** 2 + v.abs() ** 2 + w.abs() ** 2) * wp[None, :, None]).sum())
+        del u, w
+        keep = (v, phi, omy) if len(slabs) == 1 else None
+    scale = target / umax if kind == "maxu" else target / math.sqrt(esum / (3.0 * ny))
+    for sl in slabs:  # pass 2: rescaled fields, slab by slab
+        v, phi, omy = keep if keep is not None else [t for n, t in enumerate(slab(sl)) if n != 1]
+        out[0][sl].copy_(v * scale)
+        out[1][sl].copy_(phi * scale)
+        out[2][sl].copy_(omy * scale)
+        del v, phi, omy
+    keep = None
+    v, phi, omy = out
     if layout == "plane":
         v, phi, omy = (t.permute(2, 0, 1).contiguous() for t in (v, phi, omy))
     return v, phi, omy
