@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "../../include/chan.h"
+#include "chan_fft.cuh"
 #include "chan_fftkernels.cuh"
 #include "chan_plan.h"
 #include "chan_ykernels.cuh"
@@ -36,6 +37,12 @@ struct chan {
     long long nm = 0;
     int pc = 1;            // planes per FFT chunk
     int Tz = 1;            // k_x columns per z-FFT tile
+    int xthreads = 128;    // threads per row CTA of the x pass
+    void (*kzinv)(PlaneParams, FieldPtrs, int, int, double2*, int) = nullptr;
+    void (*kzfwd)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int) = nullptr;
+    void (*kx3)(PlaneParams, const double2*, int, double2*, int) = nullptr;
+    void (*kx7)(PlaneParams, const double2*, int, double2*, int) = nullptr;
+    bool zspecial = false, xspecial = false;
     // device pointers (carved)
     double2 *v, *phi, *omy, *hv, *hg, *u, *w, *ox, *oz;   // plane layout fields
     double2 *H1, *H2, *H3;                                 // alias u, w, ox
@@ -69,6 +76,7 @@ void choose_tiling(chan_t* h) {
     while (T > 1 && (size_t)P.mz * T * 16 > 112 * 1024) T >>= 1;
     while (T > 1 && T > P.nxh) T >>= 1;
     h->Tz = T;
+    h->xthreads = ((size_t)3 * P.mx * 16 > 72 * 1024) ? 256 : 128;   // <= 3 CTAs per SM: use wider CTAs
     const size_t per_plane = (size_t)13 * P.mz * P.nxh * 16;
     long long pc = (long long)(1536ull * 1024 * 1024 / per_plane);
     if (pc < 1) pc = 1;
@@ -102,7 +110,7 @@ size_t carve(chan_t* h, char* base) {
     for (int o = 0; o < 2; ++o) for (int k = 0; k < 4; ++k) h->tab[o][k] = c.take<double>(ny8 * 8);
     h->kx = c.take<double>((size_t)P.nxh * 8); h->kz = c.take<double>((size_t)P.nz * 8);
     h->wm = c.take<double>(ny8); h->wp = c.take<double>(ny8); h->wq = c.take<double>(ny8);
-    h->twx = c.take<double2>((size_t)P.mx * 16); h->twz = c.take<double2>((size_t)P.mz * 16);
+    h->twx = c.take<double2>(P.fx.tw.size() * 8); h->twz = c.take<double2>(P.fz.tw.size() * 8);
     return c.off;
 }
 
@@ -137,10 +145,12 @@ PlaneParams pparams(const chan_t* h) {
     const Plan& P = h->P;
     PlaneParams Q;
     Q.ny = P.ny; Q.nz = P.nz; Q.nxh = P.nxh; Q.nzh = P.nzh; Q.mx = P.mx; Q.mz = P.mz; Q.nm = h->nm;
-    Q.fx.n = P.mx; Q.fx.npass = (int)P.fx.radix.size(); Q.fx.tw = h->twx;
-    Q.fz.n = P.mz; Q.fz.npass = (int)P.fz.radix.size(); Q.fz.tw = h->twz;
-    for (int i = 0; i < Q.fx.npass; ++i) Q.fx.radix[i] = P.fx.radix[i];
-    for (int i = 0; i < Q.fz.npass; ++i) Q.fz.radix[i] = P.fz.radix[i];
+    auto fill = [](FftDev& D, const FftPlan& F, const double2* tw) {
+        D.n = F.n; D.ns = (int)F.radix.size();
+        for (int s = 0; s < D.ns; ++s) { D.st[s].R = F.radix[s]; D.st[s].m = F.m[s]; D.st[s].tw = tw + F.twoff[s]; }
+    };
+    fill(Q.fx, P.fx, h->twx);
+    fill(Q.fz, P.fz, h->twz);
     return Q;
 }
 
@@ -155,38 +165,73 @@ int run_derive(chan_t* h) {
     return CHAN_OK;
 }
 
-template <int T> int launch_zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
-    const size_t sm = (size_t)Q.mz * T * 16;
-    CK(cudaFuncSetAttribute(k_zfft_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    dim3 g((Q.nxh + T - 1) / T, npl, nf);
-    PB(CHAN_KC_ZFFT_INV); k_zfft_inv<T><<<g, 256, sm, h->stream>>>(Q, in, j0, npl, h->zpad); LAUNCHED();
-    return CHAN_OK;
+// ---- plan -> kernel dispatch -------------------------------------------------------------------------
+// Stage lists with kernels specialised at compile time (chan_fft.cuh k_*_s); any other list of a 2^a 3^b
+// length runs the generic kernels (k_*_g).  z lists: up to four radices; x lists: up to three radices in
+// front of the fused radix 4.
+#define CHAN_ZPLANS(X) X(6, 1, 1, 1) X(12, 1, 1, 1) X(6, 4, 1, 1) X(6, 8, 1, 1) X(12, 6, 1, 1) X(12, 8, 1, 1) X(12, 12, 1, 1) \
+    X(6, 8, 4, 1) X(6, 6, 8, 1) X(6, 8, 8, 1) X(12, 6, 8, 1) X(12, 8, 8, 1) X(12, 12, 6, 1) X(12, 12, 8, 1) X(12, 12, 12, 1) \
+    X(6, 8, 8, 4) X(6, 6, 8, 8) X(6, 8, 8, 8)
+#define CHAN_XPLANS(X) X(6, 1, 1) X(12, 1, 1) X(6, 4, 1) X(6, 6, 1) X(6, 8, 1) X(12, 8, 1) X(6, 6, 4) X(6, 6, 6) X(6, 8, 4) \
+    X(6, 6, 8) X(6, 8, 8) X(12, 6, 6) X(12, 6, 8) X(12, 8, 8)
+
+typedef void (*zinv_fn)(PlaneParams, FieldPtrs, int, int, double2*, int);
+typedef void (*zfwd_fn)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int);
+typedef void (*xprod_fn)(PlaneParams, const double2*, int, double2*, int);
+
+bool same_list(const std::vector<int>& v, int n, const int* r) {
+    int cnt = 0;
+    for (int k = 0; k < n; ++k) if (r[k] > 1) ++cnt;
+    if ((int)v.size() != cnt) return false;
+    for (int k = 0; k < cnt; ++k) if (v[k] != r[k]) return false;
+    return true;
 }
-template <int T> int launch_zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out,
-                                 double scale, int filt, int kxc, int kzc) {
-    const size_t sm = (size_t)Q.mz * T * 16;
-    CK(cudaFuncSetAttribute(k_zfft_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    dim3 g((pin + T - 1) / T, npl, nf);
-    PB(filt ? CHAN_KC_ZFFT_FWD_FILTER : CHAN_KC_ZFFT_FWD); k_zfft_fwd<T><<<g, 256, sm, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc); LAUNCHED();
-    return CHAN_OK;
-}
-int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
-    switch (h->Tz) {
-        case 16: return launch_zinv<16>(h, Q, in, nf, j0, npl);
-        case 8: return launch_zinv<8>(h, Q, in, nf, j0, npl);
-        case 4: return launch_zinv<4>(h, Q, in, nf, j0, npl);
-        case 2: return launch_zinv<2>(h, Q, in, nf, j0, npl);
-        default: return launch_zinv<1>(h, Q, in, nf, j0, npl);
+void pick_kernels(chan_t* h) {
+    const Plan& P = h->P;
+    h->kzinv = k_zfft_inv_g; h->kzfwd = k_zfft_fwd_g;
+    h->zspecial = false;
+#define X(a, b, c, d) { const int r[4] = {a, b, c, d}; if (same_list(P.fz.radix, 4, r)) { h->kzinv = k_zfft_inv_s<a, b, c, d>; h->kzfwd = k_zfft_fwd_s<a, b, c, d>; h->zspecial = true; } }
+    CHAN_ZPLANS(X)
+#undef X
+    const int F = P.fx.radix.back();
+    h->kx3 = (F == 8) ? k_xfft_prod_g<3, 8> : k_xfft_prod_g<3, 4>;
+    h->kx7 = (F == 8) ? k_xfft_prod_g<7, 8> : k_xfft_prod_g<7, 4>;
+    h->xspecial = false;
+    if (F == 4) {
+        std::vector<int> head(P.fx.radix.begin(), P.fx.radix.end() - 1);
+        if (head.empty()) { h->kx3 = k_xfft_prod_s<3, 4, 1, 1, 1>; h->kx7 = k_xfft_prod_s<7, 4, 1, 1, 1>; h->xspecial = true; }
+#define X(a, b, c) { const int r[3] = {a, b, c}; if (same_list(head, 3, r)) { h->kx3 = k_xfft_prod_s<3, 4, a, b, c>; h->kx7 = k_xfft_prod_s<7, 4, a, b, c>; h->xspecial = true; } }
+        CHAN_XPLANS(X)
+#undef X
     }
+}
+
+int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
+    const int T = h->Tz;
+    const size_t sm = (size_t)Q.mz * T * 16;
+    CK(cudaFuncSetAttribute((const void*)h->kzinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    dim3 g((Q.nxh + T - 1) / T, npl, nf);
+    PB(CHAN_KC_ZFFT_INV); h->kzinv<<<g, 256, sm, h->stream>>>(Q, in, j0, npl, h->zpad, T); LAUNCHED();
+    return CHAN_OK;
 }
 int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out, double scale, int filt, int kxc, int kzc) {
-    switch (h->Tz) {
-        case 16: return launch_zfwd<16>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
-        case 8: return launch_zfwd<8>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
-        case 4: return launch_zfwd<4>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
-        case 2: return launch_zfwd<2>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
-        default: return launch_zfwd<1>(h, Q, pin, nf, j0, npl, out, scale, filt, kxc, kzc);
-    }
+    const int T = h->Tz;
+    const size_t sm = (size_t)Q.mz * T * 16;
+    CK(cudaFuncSetAttribute((const void*)h->kzfwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    dim3 g((pin + T - 1) / T, npl, nf);
+    PB(filt ? CHAN_KC_ZFFT_FWD_FILTER : CHAN_KC_ZFFT_FWD);
+    h->kzfwd<<<g, 256, sm, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc, T); LAUNCHED();
+    return CHAN_OK;
+}
+int xprod(chan_t* h, const PlaneParams& Q, int nprod, int npl, int pout) {
+    xprod_fn fn = (nprod == 3) ? h->kx3 : h->kx7;
+    const size_t smx = (size_t)(nprod == 3 ? 3 : 4) * Q.mx * 16;
+    CK(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
+    dim3 g(Q.mz, npl);
+    PB(nprod == 3 ? CHAN_KC_XFFT_PROD : CHAN_KC_XFFT_PROD_FILTER);
+    fn<<<g, h->xthreads, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
+    LAUNCHED();
+    return CHAN_OK;
 }
 
 // a3-a8 (nprod = 3) or the product part of a13 (nprod = 7)
@@ -197,18 +242,11 @@ int run_planes(chan_t* h, int nprod, const FieldPtrsW& out, int kxc, int kzc) {
     in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w; in.f[3] = h->ox; in.f[4] = h->omy; in.f[5] = h->oz;
     const int pout = (nprod == 3) ? P.nxh : kxc + 1;
     const double scale = 1.0 / ((double)P.mx * (double)P.mz);
-    const size_t smx = (size_t)(nprod == 3 ? 3 : 4) * P.mx * 16;
-    if (nprod == 3) CK(cudaFuncSetAttribute(k_xfft_prod<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
-    else CK(cudaFuncSetAttribute(k_xfft_prod<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
     for (int j0 = 0; j0 < P.ny; j0 += h->pc) {
         const int npl = (P.ny - j0 < h->pc) ? P.ny - j0 : h->pc;
         int rc = zinv(h, Q, in, 6, j0, npl);
         if (rc) return rc;
-        dim3 g(P.mz, npl);
-        PB(nprod == 3 ? CHAN_KC_XFFT_PROD : CHAN_KC_XFFT_PROD_FILTER);
-        if (nprod == 3) k_xfft_prod<3><<<g, 256, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
-        else k_xfft_prod<7><<<g, 256, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
-        LAUNCHED();
+        if ((rc = xprod(h, Q, nprod, npl, pout))) return rc;
         rc = zfwd(h, Q, pout, nprod, j0, npl, out, scale, nprod == 7, kxc, kzc);
         if (rc) return rc;
     }
@@ -270,11 +308,12 @@ int chan_create(chan_t** out, const chan_grid_t* grid, const chan_box_t* box, do
     const int hl = opts ? opts->lhs_halfwidth : 3, hr = opts ? opts->rhs_halfwidth : 3, fo = opts ? opts->forcing : 0;
     int rc = build_plan(h->P, grid->nx, grid->ny, grid->nz, box->lx, box->lz, box->y, re_tau, dt, hl ? hl : 3, hr ? hr : 3, fo);
     if (rc != CHAN_OK) { delete h; return rc; }
-    if ((int)h->P.fx.radix.size() > CHAN_MAX_RADIX_PASSES || (int)h->P.fz.radix.size() > CHAN_MAX_RADIX_PASSES) { delete h; return CHAN_EINVAL; }
+    if ((int)h->P.fx.radix.size() > CHAN_MAX_STAGES || (int)h->P.fz.radix.size() > CHAN_MAX_STAGES) { delete h; return CHAN_EINVAL; }
     h->nm = (long long)h->P.nz * h->P.nxh;
     h->F = (size_t)h->nm * h->P.ny * 16;
     choose_tiling(h);
-    if ((size_t)3 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * 16 > 220 * 1024) { delete h; return CHAN_EINVAL; }
+    pick_kernels(h);
+    if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * 16 > 220 * 1024) { delete h; return CHAN_EINVAL; }
     h->need = carve(h, nullptr);
     *out = h;
     return CHAN_OK;

@@ -1,0 +1,536 @@
+// Wall-parallel (x,z) phase: batched plane FFTs with 3/2-rule zero padding, the pointwise products in
+// physical space and the truncation.  Steps a3-a8 and the product part of a13 of DESIGN.md
+// ("pseudo-spectral ... fully dealiased by zero padding"), L84 (batched plane FFTs), L124 (filter).
+//
+// Transform engine.  A length-n transform (n = 2^a 3^b) is a list of register-resident stages of radix
+// 2,3,4,6,8 or 12 (chan_plan.cpp chooses them), run IN PLACE in shared memory:
+//   spectral -> physical: decimation in frequency, e^{+i}, natural order in, digit-reversed order out;
+//   physical -> spectral: decimation in time, e^{-i}, the same stage list backwards.
+// Physical space is only ever used pointwise, so the digit-reversed order is never undone.
+// Stage s (radix R, sub-block m = product of the later radices, ncur = R m) owns a twiddle table
+// tw[(k-1) m + p] = exp(-2 pi i p k / ncur), k = 1..R-1, p < m, so that consecutive butterflies read
+// consecutive twiddles.  The first and last stage of a z transform read / write global memory directly
+// (padding and truncation fused); the last inverse x stage, the products and the first forward x stage are
+// one register pass.
+//
+// Every kernel body is written as `phase(ph, tid, nthreads, ...)` functions separated by barriers, all
+// __host__ __device__, so that the index algebra can be exercised on the host without a GPU.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "chan_ykernels.cuh"
+
+namespace chn {
+
+#define CHAN_MAX_STAGES 8
+
+struct FftStage {
+    int R, m;              // radix, sub-block length (product of the later radices)
+    const double2* tw;     // (R-1)*m twiddles, see above (unused when m == 1)
+};
+struct FftDev {
+    int n, ns;
+    FftStage st[CHAN_MAX_STAGES];
+};
+
+CHAN_HD c2 ldtw(const double2* p) {
+#ifdef __CUDA_ARCH__
+    const double2 v = __ldg(p);
+#else
+    const double2 v = *p;
+#endif
+    return mk(v.x, v.y);
+}
+// streaming global access: the plane data is touched once per kernel, keep it out of L1 so that the
+// twiddle tables stay there
+CHAN_HD c2 ldstream(const double2* p) {
+#ifdef __CUDA_ARCH__
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return mk(v.x, v.y);
+#else
+    return mk(p->x, p->y);
+#endif
+}
+CHAN_HD void ststream(double2* p, c2 v) {
+#ifdef __CUDA_ARCH__
+    asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+#else
+    p->x = v.x; p->y = v.y;
+#endif
+}
+
+// ---- small DFTs in registers: natural order in, natural order out; INV: e^{+i}, else e^{-i} ----------
+template <bool INV> CHAN_HD c2 rot90(c2 a) { return INV ? mk(-a.y, a.x) : mk(a.y, -a.x); }   // a*(+i) : a*(-i)
+
+template <bool INV> CHAN_HD void dft2(c2& a, c2& b) { const c2 t = a - b; a = a + b; b = t; }
+template <bool INV> CHAN_HD void dft3(c2& a0, c2& a1, c2& a2) {
+    const double s = 0.86602540378443864676;   // sin(pi/3)
+    const c2 t = a1 + a2, d = a1 - a2;
+    const c2 m = mk(a0.x - 0.5 * t.x, a0.y - 0.5 * t.y);
+    const c2 jd = rot90<INV>(mk(s * d.x, s * d.y));
+    a0 = a0 + t; a1 = m + jd; a2 = m - jd;
+}
+template <bool INV> CHAN_HD void dft4(c2& a0, c2& a1, c2& a2, c2& a3) {
+    const c2 s0 = a0 + a2, d0 = a0 - a2, s1 = a1 + a3, d1 = a1 - a3;
+    const c2 jd = rot90<INV>(d1);
+    a0 = s0 + s1; a2 = s0 - s1; a1 = d0 + jd; a3 = d0 - jd;
+}
+
+template <int R, bool INV> CHAN_HD void bfly(c2 (&a)[R]) {
+    if constexpr (R == 2) {
+        dft2<INV>(a[0], a[1]);
+    } else if constexpr (R == 3) {
+        dft3<INV>(a[0], a[1], a[2]);
+    } else if constexpr (R == 4) {
+        dft4<INV>(a[0], a[1], a[2], a[3]);
+    } else if constexpr (R == 6) {
+        // prime-factor map n = (3 n1 + 2 n2) mod 6, k = (3 k1 + 4 k2) mod 6: no internal twiddles
+        c2 A0 = a[0], A1 = a[2], A2 = a[4], B0 = a[3], B1 = a[5], B2 = a[1];
+        dft3<INV>(A0, A1, A2);
+        dft3<INV>(B0, B1, B2);
+        a[0] = A0 + B0; a[3] = A0 - B0; a[4] = A1 + B1; a[1] = A1 - B1; a[2] = A2 + B2; a[5] = A2 - B2;
+    } else if constexpr (R == 8) {
+        const double h = 0.70710678118654752440;
+        c2 s0 = a[0] + a[4], d0 = a[0] - a[4], s1 = a[1] + a[5], d1 = a[1] - a[5];
+        c2 s2 = a[2] + a[6], d2 = a[2] - a[6], s3 = a[3] + a[7], d3 = a[3] - a[7];
+        // d_n *= w8^n (forward w8 = e^{-i pi/4}; inverse its conjugate)
+        d1 = INV ? mk((d1.x - d1.y) * h, (d1.x + d1.y) * h) : mk((d1.x + d1.y) * h, (d1.y - d1.x) * h);
+        d2 = rot90<INV>(d2);
+        d3 = INV ? mk(-(d3.x + d3.y) * h, (d3.x - d3.y) * h) : mk((d3.y - d3.x) * h, -(d3.x + d3.y) * h);
+        dft4<INV>(s0, s1, s2, s3);
+        dft4<INV>(d0, d1, d2, d3);
+        a[0] = s0; a[2] = s1; a[4] = s2; a[6] = s3; a[1] = d0; a[3] = d1; a[5] = d2; a[7] = d3;
+    } else {
+        static_assert(R == 12, "unsupported radix");
+        // prime-factor map n = (4 n1 + 3 n2) mod 12, k = (4 k1 + 9 k2) mod 12: no internal twiddles
+        c2 y00 = a[0], y10 = a[4], y20 = a[8];     // n2 = 0
+        c2 y01 = a[3], y11 = a[7], y21 = a[11];    // n2 = 1
+        c2 y02 = a[6], y12 = a[10], y22 = a[2];    // n2 = 2
+        c2 y03 = a[9], y13 = a[1], y23 = a[5];     // n2 = 3
+        dft3<INV>(y00, y10, y20); dft3<INV>(y01, y11, y21); dft3<INV>(y02, y12, y22); dft3<INV>(y03, y13, y23);
+        dft4<INV>(y00, y01, y02, y03);             // k1 = 0 -> k = 0, 9, 6, 3
+        dft4<INV>(y10, y11, y12, y13);             // k1 = 1 -> k = 4, 1, 10, 7
+        dft4<INV>(y20, y21, y22, y23);             // k1 = 2 -> k = 8, 5, 2, 11
+        a[0] = y00; a[9] = y01; a[6] = y02; a[3] = y03;
+        a[4] = y10; a[1] = y11; a[10] = y12; a[7] = y13;
+        a[8] = y20; a[5] = y21; a[2] = y22; a[11] = y23;
+    }
+}
+
+// One butterfly of an in-place pass: elements base + k m, k < R, of sequence q.
+//   DIF (inverse direction here): butterfly, then output k times conj(w^k);
+//   DIT (forward direction here): input k times w^k, then butterfly.     w[k-1] = table twiddle (e^{-i}).
+template <int R, bool INV, bool DIT, class Src, class Dst>
+CHAN_HD void pass_item(const Src& src, const Dst& dst, int q, int base, int m, const c2 (&w)[R - 1 > 0 ? R - 1 : 1], bool twiddled) {
+    c2 a[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) a[k] = src.load(base + k * m, q);
+    if (DIT && twiddled) {
+#pragma unroll
+        for (int k = 1; k < R; ++k) a[k] = cmul(a[k], INV ? mk(w[k - 1].x, -w[k - 1].y) : w[k - 1]);
+    }
+    bfly<R, INV>(a);
+    if (!DIT && twiddled) {
+#pragma unroll
+        for (int k = 1; k < R; ++k) a[k] = cmul(a[k], INV ? mk(w[k - 1].x, -w[k - 1].y) : w[k - 1]);
+    }
+#pragma unroll
+    for (int k = 0; k < R; ++k) dst.store(base + k * m, q, a[k]);
+}
+
+struct PlaneParams {
+    int ny, nz, nxh, nzh, mx, mz;
+    long long nm;          // nz*nxh
+    FftDev fx, fz;
+};
+struct FieldPtrs { const double2* f[8]; };
+struct FieldPtrsW { double2* f[8]; };
+
+// =====================================================================================================
+// z transforms: tile of T k_x columns, shared layout [e][T] (column fastest).  Work item = (butterfly b,
+// column t), t fastest over the lanes: every shared access of 8 lanes is one contiguous 128-byte row and
+// the twiddle of a butterfly is a broadcast load.
+// =====================================================================================================
+template <int R, bool INV, bool DIT, class Src, class Dst>
+CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int T, int tid, int nt) {
+    const int m = S.m, ncur = R * m, nb = n / R;
+    const int total = nb * T;
+    for (int w = tid; w < total; w += nt) {
+        const int b = w / T, t = w - b * T;     // T is a power of two
+        const int blk = b / m, p = b - blk * m;
+        c2 tw[R - 1 > 0 ? R - 1 : 1];
+        if (m > 1) {
+#pragma unroll
+            for (int k = 1; k < R; ++k) tw[k - 1] = ldtw(S.tw + (size_t)(k - 1) * m + p);
+        }
+        pass_item<R, INV, DIT>(src, dst, t, blk * ncur + p, m, tw, m > 1);
+    }
+}
+template <bool INV, bool DIT, class Src, class Dst>
+CHAN_HD void zpass_any(const Src& src, const Dst& dst, const FftStage& S, int n, int T, int tid, int nt) {
+    switch (S.R) {
+        case 2: zpass<2, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+        case 3: zpass<3, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+        case 4: zpass<4, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+        case 6: zpass<6, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+        case 8: zpass<8, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+        default: zpass<12, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+    }
+}
+
+// ---- K2 (a3): zero-pad in k_z, inverse c2c along z -------------------------------------------------
+// in: plane-layout field (rows s = k_z slot, nz of them); out: zpad[f][jc][r][p], r = position in the
+// digit-reversed physical z order.
+struct ZInvIO {
+    c2* sm; int T;
+    bool gin, gout;                 // this stage reads / writes global memory
+    const double2* src;             // plane of the field: [nz][nxh]
+    double2* dst;                   // plane of zpad: [mz][nxh]
+    int nxh, nzh, nz, mz, p0, tcount;
+    CHAN_HD c2 load(int e, int t) const {
+        if (!gin) return sm[e * T + t];
+        int s = -1;
+        if (e < nzh) s = e; else if (e > mz - nzh) s = e - (mz - nz);
+        return (s >= 0 && t < tcount) ? ldstream(src + (size_t)s * nxh + p0 + t) : mk(0, 0);
+    }
+    CHAN_HD void store(int e, int t, c2 v) const {
+        if (!gout) { sm[e * T + t] = v; return; }
+        if (t < tcount) ststream(dst + (size_t)e * nxh + p0 + t, v);
+    }
+};
+CHAN_HD void zinv_phase(int ph, int tid, int nt, const PlaneParams& P, int T, c2* sm, const double2* src, double2* dst, int p0) {
+    ZInvIO io;
+    io.sm = sm; io.T = T; io.gin = (ph == 0); io.gout = (ph == P.fz.ns - 1);
+    io.src = src; io.dst = dst; io.nxh = P.nxh; io.nzh = P.nzh; io.nz = P.nz; io.mz = P.mz; io.p0 = p0;
+    io.tcount = (P.nxh - p0 < T) ? P.nxh - p0 : T;
+    zpass_any<true, false>(io, io, P.fz.st[ph], P.mz, T, tid, nt);
+}
+
+// ---- K4 (a7-a8): forward c2c along z, truncate, scale ----------------------------------------------
+//   filt 0: retained modes into plane-layout fields (Nyquist slot zeroed), all p < pin = nxh;
+//   filt 1: |q| <= kzc, p <= kxc into out[j][2kzc+1][kxc+1].
+// in: xh[f][jc][r][pin].
+struct ZFwdIO {
+    c2* sm; int T;
+    bool gin, gout;
+    const double2* src;             // plane of xh: [mz][pin]
+    double2* dst;                   // filt 0: plane [nz][nxh]; filt 1: plane [2kzc+1][kxc+1]
+    int pin, nxh, nzh, nz, mz, p0, tcount, filt, kxc, kzc;
+    double scale;
+    CHAN_HD c2 load(int e, int t) const {
+        if (!gin) return sm[e * T + t];
+        return (t < tcount) ? ldstream(src + (size_t)e * pin + p0 + t) : mk(0, 0);
+    }
+    CHAN_HD void store(int e, int t, c2 v) const {
+        if (!gout) { sm[e * T + t] = v; return; }
+        if (t >= tcount) return;
+        if (!filt) {
+            int s;
+            if (e < nzh) s = e; else if (e > mz - nzh) s = e - (mz - nz); else if (e == nzh) { s = nzh; v = mk(0, 0); } else return;
+            ststream(dst + (size_t)s * nxh + p0 + t, mk(v.x * scale, v.y * scale));
+        } else {
+            const int nr = 2 * kzc + 1, npk = kxc + 1;
+            int rr;
+            if (e <= kzc) rr = e; else if (e >= mz - kzc) rr = e - mz + nr; else return;
+            if (p0 + t < npk) ststream(dst + (size_t)rr * npk + p0 + t, mk(v.x * scale, v.y * scale));
+        }
+    }
+};
+CHAN_HD void zfwd_phase(int ph, int tid, int nt, const PlaneParams& P, int T, c2* sm, const double2* src, double2* dst, int pin,
+                        int p0, double scale, int filt, int kxc, int kzc) {
+    ZFwdIO io;
+    io.sm = sm; io.T = T; io.gin = (ph == 0); io.gout = (ph == P.fz.ns - 1);
+    io.src = src; io.dst = dst; io.pin = pin; io.nxh = P.nxh; io.nzh = P.nzh; io.nz = P.nz; io.mz = P.mz; io.p0 = p0;
+    io.tcount = (pin - p0 < T) ? pin - p0 : T;
+    io.filt = filt; io.kxc = kxc; io.kzc = kzc; io.scale = scale;
+    zpass_any<false, true>(io, io, P.fz.st[P.fz.ns - 1 - ph], P.mz, T, tid, nt);
+}
+
+// Kernels.  k_z*_g: any stage list (run-time radix switch; correct for every 2^a 3^b length but the
+// compiler keeps the registers of all radices alive).  k_z*_s<R0..R3>: the same phases with the stage
+// radices as template parameters (R = 1: absent) -- the plans chan_api.cu dispatches to.
+CHAN_HD ZInvIO make_zinv_io(const PlaneParams& P, int T, c2* sm, const double2* src, double2* dst, int p0) {
+    ZInvIO io;
+    io.sm = sm; io.T = T; io.gin = false; io.gout = false;
+    io.src = src; io.dst = dst; io.nxh = P.nxh; io.nzh = P.nzh; io.nz = P.nz; io.mz = P.mz; io.p0 = p0;
+    io.tcount = (P.nxh - p0 < T) ? P.nxh - p0 : T;
+    return io;
+}
+CHAN_HD ZFwdIO make_zfwd_io(const PlaneParams& P, int T, c2* sm, const double2* src, double2* dst, int pin, int p0, double scale,
+                            int filt, int kxc, int kzc) {
+    ZFwdIO io;
+    io.sm = sm; io.T = T; io.gin = false; io.gout = false;
+    io.src = src; io.dst = dst; io.pin = pin; io.nxh = P.nxh; io.nzh = P.nzh; io.nz = P.nz; io.mz = P.mz; io.p0 = p0;
+    io.tcount = (pin - p0 < T) ? pin - p0 : T;
+    io.filt = filt; io.kxc = kxc; io.kzc = kzc; io.scale = scale;
+    return io;
+}
+
+#ifdef __CUDACC__
+#define CHAN_ZARGS_INV PlaneParams P, FieldPtrs in, int j0, int npl, double2* __restrict__ zpad, int T
+#define CHAN_ZARGS_FWD PlaneParams P, const double2* __restrict__ xh, int pin, int j0, int npl, FieldPtrsW out, double scale, int filt, int kxc, int kzc, int T
+
+__global__ void __launch_bounds__(256, 2) k_zfft_inv_g(CHAN_ZARGS_INV) {
+    extern __shared__ double2 smem_raw[];
+    c2* sm = reinterpret_cast<c2*>(smem_raw);
+    const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
+    const double2* src = in.f[fi] + (size_t)(j0 + jc) * P.nm;
+    double2* dst = zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh;
+#pragma unroll 1
+    for (int ph = 0; ph < P.fz.ns; ++ph) {
+        if (ph) __syncthreads();
+        zinv_phase(ph, threadIdx.x, blockDim.x, P, T, sm, src, dst, p0);
+    }
+}
+__global__ void __launch_bounds__(256, 2) k_zfft_fwd_g(CHAN_ZARGS_FWD) {
+    extern __shared__ double2 smem_raw[];
+    c2* sm = reinterpret_cast<c2*>(smem_raw);
+    const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
+    const int j = j0 + jc;
+    const double2* src = xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin;
+    double2* dst = filt ? out.f[fi] + (size_t)j * (2 * kzc + 1) * (kxc + 1) : out.f[fi] + (size_t)j * P.nm;
+#pragma unroll 1
+    for (int ph = 0; ph < P.fz.ns; ++ph) {
+        if (ph) __syncthreads();
+        zfwd_phase(ph, threadIdx.x, blockDim.x, P, T, sm, src, dst, pin, p0, scale, filt, kxc, kzc);
+    }
+}
+
+template <int R0, int R1, int R2, int R3>
+__global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
+    extern __shared__ double2 smem_raw[];
+    constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
+    const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
+    ZInvIO io = make_zinv_io(P, T, reinterpret_cast<c2*>(smem_raw), in.f[fi] + (size_t)(j0 + jc) * P.nm,
+                             zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
+    const int tid = threadIdx.x, nt = blockDim.x, mz = P.mz;
+    io.gin = true; io.gout = (NS == 1);
+    zpass<R0, true, false>(io, io, P.fz.st[0], mz, T, tid, nt);
+    if constexpr (NS > 1) {
+        __syncthreads();
+        io.gin = false; io.gout = (NS == 2);
+        zpass<R1, true, false>(io, io, P.fz.st[1], mz, T, tid, nt);
+    }
+    if constexpr (NS > 2) {
+        __syncthreads();
+        io.gout = (NS == 3);
+        zpass<R2, true, false>(io, io, P.fz.st[2], mz, T, tid, nt);
+    }
+    if constexpr (NS > 3) {
+        __syncthreads();
+        io.gout = true;
+        zpass<R3, true, false>(io, io, P.fz.st[3], mz, T, tid, nt);
+    }
+}
+template <int R0, int R1, int R2, int R3>
+__global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
+    extern __shared__ double2 smem_raw[];
+    constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
+    const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
+    const int j = j0 + jc;
+    ZFwdIO io = make_zfwd_io(P, T, reinterpret_cast<c2*>(smem_raw), xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin,
+                             filt ? out.f[fi] + (size_t)j * (2 * kzc + 1) * (kxc + 1) : out.f[fi] + (size_t)j * P.nm, pin, p0, scale,
+                             filt, kxc, kzc);
+    const int tid = threadIdx.x, nt = blockDim.x, mz = P.mz;
+    io.gin = true;
+    if constexpr (NS > 3) {
+        zpass<R3, false, true>(io, io, P.fz.st[3], mz, T, tid, nt);
+        __syncthreads();
+        io.gin = false;
+    }
+    if constexpr (NS > 2) {
+        zpass<R2, false, true>(io, io, P.fz.st[2], mz, T, tid, nt);
+        __syncthreads();
+        io.gin = false;
+    }
+    if constexpr (NS > 1) {
+        zpass<R1, false, true>(io, io, P.fz.st[1], mz, T, tid, nt);
+        __syncthreads();
+        io.gin = false;
+    }
+    io.gout = true;
+    zpass<R0, false, true>(io, io, P.fz.st[0], mz, T, tid, nt);
+}
+#endif
+
+// =====================================================================================================
+// x transforms (K3, a4-a6): one (plane, z) row per CTA.  Six spectral rows are packed into three complex
+// sequences (A + iB with A, B Hermitian), inverse transformed, multiplied pointwise, and the products go
+// back as packed forward transforms.  Shared layout [sequence][swz(e)] with
+// swz(e) = e ^ ((e >> 3) & 7): contiguous runs of 8, stride-4 and stride-8 butterflies are all free of
+// bank conflicts for 16-byte elements.  One thread owns butterfly b of EVERY sequence, so the twiddles
+// are loaded once per butterfly and reused.
+//   NPROD = 3: H = u x omega (reading R1).   NPROD = 7: uu,uv,uw,vv,vw,ww, om.om (filter, R12).
+// zpad fields in order u,v,w,om_x,om_y,om_z.
+// =====================================================================================================
+CHAN_HD int swz(int e) { return e ^ ((e >> 3) & 7); }
+struct XIO {
+    c2* sm; int stride;
+    CHAN_HD c2 load(int e, int q) const { return sm[q * stride + swz(e)]; }
+    CHAN_HD void store(int e, int q, c2 v) const { sm[q * stride + swz(e)] = v; }
+};
+template <int R, bool INV, bool DIT>
+CHAN_HD void xpass(const XIO& io, const FftStage& S, int n, int nseq, int tid, int nt) {
+    const int m = S.m, ncur = R * m, nb = n / R;
+    for (int b = tid; b < nb; b += nt) {
+        const int blk = b / m, p = b - blk * m;
+        c2 tw[R - 1];
+        if (m > 1) {
+#pragma unroll
+            for (int k = 1; k < R; ++k) tw[k - 1] = ldtw(S.tw + (size_t)(k - 1) * m + p);
+        }
+        for (int q = 0; q < nseq; ++q) pass_item<R, INV, DIT>(io, io, q, blk * ncur + p, m, tw, m > 1);
+    }
+}
+template <bool INV, bool DIT>
+CHAN_HD void xpass_any(const XIO& io, const FftStage& S, int n, int nseq, int tid, int nt) {
+    switch (S.R) {
+        case 2: xpass<2, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        case 3: xpass<3, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        case 4: xpass<4, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        case 6: xpass<6, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        case 8: xpass<8, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        default: xpass<12, INV, DIT>(io, S, n, nseq, tid, nt); break;
+    }
+}
+
+// last inverse stage (radix F, m = 1, no twiddles) + products + first forward stage, in registers
+template <int F, int NPROD>
+CHAN_HD void xfused(const XIO& io, int n, int tid, int nt) {
+    for (int b = tid; b < n / F; b += nt) {
+        c2 s0[F], s1[F], s2[F];
+#pragma unroll
+        for (int k = 0; k < F; ++k) { s0[k] = io.load(F * b + k, 0); s1[k] = io.load(F * b + k, 1); s2[k] = io.load(F * b + k, 2); }
+        bfly<F, true>(s0); bfly<F, true>(s1); bfly<F, true>(s2);
+        // s0 = u + i v, s1 = w + i om_x, s2 = om_y + i om_z at F physical points
+        if constexpr (NPROD == 3) {
+            c2 o[F];
+#pragma unroll
+            for (int k = 0; k < F; ++k) o[k] = mk(s0[k].y * s2[k].y - s1[k].x * s2[k].x, s1[k].x * s1[k].y - s0[k].x * s2[k].y);
+            bfly<F, false>(o);
+#pragma unroll
+            for (int k = 0; k < F; ++k) io.store(F * b + k, 0, o[k]);
+#pragma unroll
+            for (int k = 0; k < F; ++k) o[k] = mk(s0[k].x * s2[k].x - s0[k].y * s1[k].y, 0.0);
+            bfly<F, false>(o);
+#pragma unroll
+            for (int k = 0; k < F; ++k) io.store(F * b + k, 1, o[k]);
+        } else {
+            c2 o[F];
+#pragma unroll
+            for (int k = 0; k < F; ++k) o[k] = mk(s0[k].x * s0[k].x, s0[k].x * s0[k].y);
+            bfly<F, false>(o);
+#pragma unroll
+            for (int k = 0; k < F; ++k) io.store(F * b + k, 0, o[k]);
+#pragma unroll
+            for (int k = 0; k < F; ++k) o[k] = mk(s0[k].x * s1[k].x, s0[k].y * s0[k].y);
+            bfly<F, false>(o);
+#pragma unroll
+            for (int k = 0; k < F; ++k) io.store(F * b + k, 1, o[k]);
+#pragma unroll
+            for (int k = 0; k < F; ++k) o[k] = mk(s0[k].y * s1[k].x, s1[k].x * s1[k].x);
+            bfly<F, false>(o);
+#pragma unroll
+            for (int k = 0; k < F; ++k) io.store(F * b + k, 2, o[k]);
+#pragma unroll
+            for (int k = 0; k < F; ++k) o[k] = mk(s1[k].y * s1[k].y + s2[k].x * s2[k].x + s2[k].y * s2[k].y, 0.0);
+            bfly<F, false>(o);
+#pragma unroll
+            for (int k = 0; k < F; ++k) io.store(F * b + k, 3, o[k]);
+        }
+    }
+}
+
+CHAN_HD void xpack(const XIO& io, int mx, int nxh, const double2* zrow, size_t fstride, int tid, int nt) {
+    // C[k] = A[k] + i B[k], C[mx-k] = conj(A[k]) + i conj(B[k]); Im of the k = 0 entries dropped (R14)
+    for (int w = tid; w < 3 * nxh; w += nt) {
+        const int pr = w / nxh, k = w - pr * nxh;
+        const c2 A = ldstream(zrow + (size_t)(2 * pr) * fstride + k), B = ldstream(zrow + (size_t)(2 * pr + 1) * fstride + k);
+        if (k == 0) io.store(0, pr, mk(A.x, B.x));
+        else { io.store(k, pr, mk(A.x - B.y, A.y + B.x)); io.store(mx - k, pr, mk(A.x + B.y, -A.y + B.x)); }
+    }
+    const int nzero = mx - 2 * nxh + 1;     // entries nxh .. mx-nxh
+    for (int w = tid; w < 3 * nzero; w += nt) {
+        const int pr = w / nzero, k = w - pr * nzero;
+        io.store(nxh + k, pr, mk(0, 0));
+    }
+}
+template <int NPROD>
+CHAN_HD void xunpack(const XIO& io, int mx, double2* xrow, size_t ostride, int pout, int tid, int nt) {
+    constexpr int NC = (NPROD + 1) / 2;
+    // A[k] = (D[k] + conj D[mx-k])/2, B[k] = (D[k] - conj D[mx-k])/(2i)
+    for (int w = tid; w < NC * pout; w += nt) {
+        const int pr = w / pout, k = w - pr * pout;
+        const c2 d = io.load(k, pr), e = io.load(k == 0 ? 0 : mx - k, pr);
+        ststream(xrow + (size_t)(2 * pr) * ostride + k, mk(0.5 * (d.x + e.x), 0.5 * (d.y - e.y)));
+        if (2 * pr + 1 < NPROD) ststream(xrow + (size_t)(2 * pr + 1) * ostride + k, mk(0.5 * (d.y + e.y), -0.5 * (d.x - e.x)));
+    }
+}
+
+// Phases of one row: 0 pack | 1..ns-1 inverse stages 0..ns-2 | ns fused | ns+1..2ns-1 forward stages
+// ns-2..0 | 2ns unpack.   zrow: row (jc, r) of the six zpad fields (field stride fstride);
+// xrow: row of the NPROD xh fields (field stride ostride, row pitch pout).
+template <int NPROD, int F>
+CHAN_HD void xrow_phase(int ph, int tid, int nt, const PlaneParams& P, c2* sm, const double2* zrow, size_t fstride,
+                        double2* xrow, size_t ostride, int pout) {
+    constexpr int NC = (NPROD + 1) / 2;
+    const int mx = P.mx, nxh = P.nxh, ns = P.fx.ns;
+    XIO io; io.sm = sm; io.stride = mx;
+    if (ph == 0) {
+        xpack(io, mx, nxh, zrow, fstride, tid, nt);
+    } else if (ph < ns) {
+        xpass_any<true, false>(io, P.fx.st[ph - 1], mx, 3, tid, nt);
+    } else if (ph == ns) {
+        xfused<F, NPROD>(io, mx, tid, nt);
+    } else if (ph < 2 * ns) {
+        xpass_any<false, true>(io, P.fx.st[2 * ns - 1 - ph], mx, NC, tid, nt);
+    } else {
+        xunpack<NPROD>(io, mx, xrow, ostride, pout, tid, nt);
+    }
+}
+
+#ifdef __CUDACC__
+#define CHAN_XARGS PlaneParams P, const double2* __restrict__ zpad, int npl, double2* __restrict__ xh, int pout
+
+// any stage list (run-time radix switch)
+template <int NPROD, int F>
+__global__ void __launch_bounds__(256, 2) k_xfft_prod_g(CHAN_XARGS) {
+    extern __shared__ double2 smem_raw[];
+    c2* sm = reinterpret_cast<c2*>(smem_raw);    // [max(3, NC)][mx]
+    const int r = blockIdx.x, jc = blockIdx.y;
+    const size_t fstride = (size_t)npl * P.mz * P.nxh;
+    const double2* zrow = zpad + ((size_t)jc * P.mz + r) * P.nxh;
+    const size_t ostride = (size_t)npl * P.mz * pout;
+    double2* xrow = xh + ((size_t)jc * P.mz + r) * pout;
+    const int nph = 2 * P.fx.ns + 1;
+#pragma unroll 1
+    for (int ph = 0; ph < nph; ++ph) {
+        if (ph) __syncthreads();
+        xrow_phase<NPROD, F>(ph, threadIdx.x, blockDim.x, P, sm, zrow, fstride, xrow, ostride, pout);
+    }
+}
+
+// stage radices as template parameters: R0, R1, R2 (1 = absent) then the fused radix F
+template <int NPROD, int F, int R0, int R1, int R2>
+__global__ void __launch_bounds__(256, 2) k_xfft_prod_s(CHAN_XARGS) {
+    extern __shared__ double2 smem_raw[];
+    constexpr int NC = (NPROD + 1) / 2;
+    const int r = blockIdx.x, jc = blockIdx.y;
+    const int tid = threadIdx.x, nt = blockDim.x, mx = P.mx;
+    XIO io; io.sm = reinterpret_cast<c2*>(smem_raw); io.stride = mx;
+    xpack(io, mx, P.nxh, zpad + ((size_t)jc * P.mz + r) * P.nxh, (size_t)npl * P.mz * P.nxh, tid, nt);
+    __syncthreads();
+    if constexpr (R0 > 1) { xpass<R0, true, false>(io, P.fx.st[0], mx, 3, tid, nt); __syncthreads(); }
+    if constexpr (R1 > 1) { xpass<R1, true, false>(io, P.fx.st[1], mx, 3, tid, nt); __syncthreads(); }
+    if constexpr (R2 > 1) { xpass<R2, true, false>(io, P.fx.st[2], mx, 3, tid, nt); __syncthreads(); }
+    xfused<F, NPROD>(io, mx, tid, nt);
+    __syncthreads();
+    if constexpr (R2 > 1) { xpass<R2, false, true>(io, P.fx.st[2], mx, NC, tid, nt); __syncthreads(); }
+    if constexpr (R1 > 1) { xpass<R1, false, true>(io, P.fx.st[1], mx, NC, tid, nt); __syncthreads(); }
+    if constexpr (R0 > 1) { xpass<R0, false, true>(io, P.fx.st[0], mx, NC, tid, nt); __syncthreads(); }
+    xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
+}
+#endif
+
+}  // namespace chn

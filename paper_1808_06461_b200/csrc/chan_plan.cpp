@@ -11,6 +11,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "../../include/chan.h"
@@ -163,26 +164,72 @@ void pad8(int ny, const std::vector<double>& T, std::vector<double>& O) {
     for (int i = 0; i < ny; ++i) for (int k = 0; k < 7; ++k) O[(size_t)i * 8 + k] = T[(size_t)i * 7 + k];
 }
 
-bool make_fft_plan(int n, FftPlan& F) {
-    F.n = n;
-    F.radix.clear();
-    int r = n;
-    std::vector<int> twos, threes;
-    while (r % 3 == 0) { threes.push_back(3); r /= 3; }
-    int p2 = 0;
-    while (r % 2 == 0) { ++p2; r /= 2; }
-    if (r != 1 || n < 2) return false;
-    for (; p2 >= 2; p2 -= 2) F.radix.push_back(4);
-    if (p2) F.radix.push_back(2);
-    for (int t : threes) F.radix.push_back(t);
-    F.tw.resize((size_t)2 * n);
-    const ld two_pi = 6.283185307179586476925286766559005768L;
-    for (int k = 0; k < n; ++k) {
-        // exact octant reduction keeps the table symmetric to the last bit
-        ld a = two_pi * (ld)k / (ld)n;
-        F.tw[2 * k] = (double)cosl(a);
-        F.tw[2 * k + 1] = (double)(-sinl(a));
+// Stage list for length n = 2^a 3^b (chan_fft.cuh).  `fused_last` > 0 fixes the last radix (the x
+// transform fuses that stage with the pointwise products); the rest is the shortest list of radices from
+// {12,8,6,4,3,2} (fewest radix-12 stages among the shortest), radices with a factor 3 first so that the
+// zero band of the 3/2 padding lines up with whole inputs of the first butterfly.
+void best_radices(int rest, int maxr, std::vector<int>& cur, std::vector<int>& best) {
+    static const int cand[6] = {12, 8, 6, 4, 3, 2};
+    if (rest == 1) {
+        auto key = [](const std::vector<int>& v) {
+            int c12 = 0, c2 = 0;
+            for (int r : v) { c12 += (r == 12); c2 += (r <= 3); }
+            return (long)v.size() * 10000 + c12 * 100 + c2;
+        };
+        if (best.empty() || key(cur) < key(best)) best = cur;
+        return;
     }
+    if (!best.empty() && cur.size() + 1 > best.size()) return;
+    for (int r : cand) {
+        if (r > maxr || rest % r) continue;
+        if (!cur.empty() && r > cur.back()) continue;   // non-increasing: each multiset once
+        cur.push_back(r);
+        best_radices(rest / r, maxr, cur, best);
+        cur.pop_back();
+    }
+}
+
+bool make_fft_plan(int n, int fused_last, int maxr, FftPlan& F) {
+    F.n = n;
+    F.radix.clear(); F.m.clear(); F.twoff.clear(); F.tw.clear();
+    int r = n;
+    while (r % 3 == 0) r /= 3;
+    while (r % 2 == 0) r /= 2;
+    if (r != 1 || n < 2) return false;
+    int rest = n;
+    if (fused_last > 0) {
+        if (n % fused_last) return false;
+        rest = n / fused_last;
+    }
+    std::vector<int> cur, best;
+    if (rest > 1) {
+        best_radices(rest, maxr, cur, best);
+        if (best.empty()) return false;
+    }
+    std::stable_sort(best.begin(), best.end(), [](int a, int b) {
+        const int a3 = (a % 3 == 0), b3 = (b % 3 == 0);
+        return a3 != b3 ? a3 > b3 : a > b;
+    });
+    F.radix = best;
+    if (fused_last > 0) F.radix.push_back(fused_last);
+    const ld two_pi = 6.283185307179586476925286766559005768L;
+    int m = n;
+    for (size_t s = 0; s < F.radix.size(); ++s) {
+        const int R = F.radix[s];
+        m /= R;
+        F.m.push_back(m);
+        F.twoff.push_back(F.tw.size() / 2);
+        if (m == 1) continue;
+        const long ncur = (long)R * m;
+        for (int k = 1; k < R; ++k)
+            for (int p = 0; p < m; ++p) {
+                const long e = ((long)p * k) % ncur;
+                const ld a = two_pi * (ld)e / (ld)ncur;
+                F.tw.push_back((double)cosl(a));
+                F.tw.push_back((double)(-sinl(a)));
+            }
+    }
+    if (F.tw.empty()) { F.tw.push_back(1.0); F.tw.push_back(0.0); }
     return true;
 }
 
@@ -199,7 +246,13 @@ int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const doub
     P.lx = lx; P.lz = lz; P.nu = 1.0 / re_tau; P.dt = dt;
     P.half_lhs = half_lhs; P.half_rhs = half_rhs; P.forcing = forcing;
     P.y.assign(y, y + ny);
-    if (!make_fft_plan(P.mx, P.fx) || !make_fft_plan(P.mz, P.fz)) return CHAN_EINVAL;
+    // x: the last stage is fused with the products and needs the 8-aligned swizzle of chan_fft.cuh
+    if (P.mx % 8) return CHAN_EINVAL;
+    const char* ef = std::getenv("CHAN_XFUSE");
+    const char* er = std::getenv("CHAN_MAXRADIX");
+    const int fuse = (ef && std::atoi(ef) == 8) ? 8 : 4;
+    const int maxr = (er && std::atoi(er) >= 2) ? std::atoi(er) : 12;
+    if (!make_fft_plan(P.mx, fuse, maxr, P.fx) || !make_fft_plan(P.mz, 0, maxr, P.fz)) return CHAN_EINVAL;
 
     // RK3 constants of [34] (reading R3)
     const double al[3] = {29.0 / 96.0, -3.0 / 40.0, 1.0 / 6.0}, be[3] = {37.0 / 160.0, 5.0 / 24.0, 1.0 / 6.0};

@@ -2,14 +2,20 @@
 // Everything here is computed in long double on the host, independently of the oracle
 // (include/chan.h; readings R2-R5).
 #pragma once
+#include <cstddef>
 #include <vector>
 
 namespace chn {
 
+// Stage list of one transform length (chan_fft.cuh): stage s has radix[s] and sub-block length
+// m[s] = product of the later radices; its twiddles exp(-2 pi i p k/(radix m)), k = 1..radix-1, p < m,
+// start at complex offset twoff[s] of tw, laid out [(k-1) m + p].
 struct FftPlan {
     int n = 0;
     std::vector<int> radix;     // DIF order (largest sub-transform first); DIT runs it backwards
-    std::vector<double> tw;     // n complex twiddles exp(-2 pi i k / n), interleaved re,im
+    std::vector<int> m;
+    std::vector<size_t> twoff;
+    std::vector<double> tw;     // interleaved re,im
 };
 
 // Row-constant tables for one orientation (0 = natural y order, 1 = flipped, i -> ny-1-i).

@@ -13,15 +13,16 @@
 
 namespace chn {
 
+#define CHAN_HD __host__ __device__ __forceinline__
 struct c2 { double x, y; };
-__device__ __forceinline__ c2 mk(double a, double b) { c2 r; r.x = a; r.y = b; return r; }
-__device__ __forceinline__ c2 operator+(c2 a, c2 b) { return mk(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ c2 operator-(c2 a, c2 b) { return mk(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ c2 operator*(double s, c2 a) { return mk(s * a.x, s * a.y); }
-__device__ __forceinline__ c2 cmul(c2 a, c2 b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ c2 muli(c2 a) { return mk(-a.y, a.x); }  // i * a
-__device__ __forceinline__ c2 ldc(const double2* p) { double2 v = *p; return mk(v.x, v.y); }
-__device__ __forceinline__ void stc(double2* p, c2 v) { *p = make_double2(v.x, v.y); }
+CHAN_HD c2 mk(double a, double b) { c2 r; r.x = a; r.y = b; return r; }
+CHAN_HD c2 operator+(c2 a, c2 b) { return mk(a.x + b.x, a.y + b.y); }
+CHAN_HD c2 operator-(c2 a, c2 b) { return mk(a.x - b.x, a.y - b.y); }
+CHAN_HD c2 operator*(double s, c2 a) { return mk(s * a.x, s * a.y); }
+CHAN_HD c2 cmul(c2 a, c2 b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+CHAN_HD c2 muli(c2 a) { return mk(-a.y, a.x); }  // i * a
+CHAN_HD c2 ldc(const double2* p) { double2 v = *p; return mk(v.x, v.y); }
+CHAN_HD void stc(double2* p, c2 v) { *p = make_double2(v.x, v.y); }
 
 struct YTab {               // device pointers to the row tables of one orientation
     const double* B1;       // [ny][8]
