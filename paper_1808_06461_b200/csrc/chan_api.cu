@@ -168,12 +168,13 @@ int run_derive(chan_t* h) {
 // ---- plan -> kernel dispatch -------------------------------------------------------------------------
 // Stage lists with kernels specialised at compile time (chan_fft.cuh k_*_s); any other list of a 2^a 3^b
 // length runs the generic kernels (k_*_g).  z lists: up to four radices; x lists: up to three radices in
-// front of the fused radix 4.
+// front of the fused radix (4 or 8).
 #define CHAN_ZPLANS(X) X(6, 1, 1, 1) X(12, 1, 1, 1) X(6, 4, 1, 1) X(6, 8, 1, 1) X(12, 6, 1, 1) X(12, 8, 1, 1) X(12, 12, 1, 1) \
     X(6, 8, 4, 1) X(6, 6, 8, 1) X(6, 8, 8, 1) X(12, 6, 8, 1) X(12, 8, 8, 1) X(12, 12, 6, 1) X(12, 12, 8, 1) X(12, 12, 12, 1) \
     X(6, 8, 8, 4) X(6, 6, 8, 8) X(6, 8, 8, 8)
-#define CHAN_XPLANS(X) X(6, 1, 1) X(12, 1, 1) X(6, 4, 1) X(6, 6, 1) X(6, 8, 1) X(12, 8, 1) X(6, 6, 4) X(6, 6, 6) X(6, 8, 4) \
-    X(6, 6, 8) X(6, 8, 8) X(12, 6, 6) X(12, 6, 8) X(12, 8, 8)
+#define CHAN_XPLANS(X) X(4, 6, 1, 1) X(4, 12, 1, 1) X(4, 6, 4, 1) X(4, 6, 6, 1) X(4, 6, 8, 1) X(4, 12, 8, 1) X(4, 6, 6, 4) X(4, 6, 6, 6) \
+    X(4, 6, 8, 4) X(4, 6, 6, 8) X(4, 6, 8, 8) X(4, 12, 6, 6) X(4, 12, 6, 8) X(4, 12, 8, 8) X(8, 6, 1, 1) X(8, 12, 1, 1) X(8, 12, 6, 1) \
+    X(8, 12, 12, 1) X(8, 6, 8, 1)
 
 typedef void (*zinv_fn)(PlaneParams, FieldPtrs, int, int, double2*, int);
 typedef void (*zfwd_fn)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int);
@@ -197,10 +198,11 @@ void pick_kernels(chan_t* h) {
     h->kx3 = (F == 8) ? k_xfft_prod_g<3, 8> : k_xfft_prod_g<3, 4>;
     h->kx7 = (F == 8) ? k_xfft_prod_g<7, 8> : k_xfft_prod_g<7, 4>;
     h->xspecial = false;
-    if (F == 4) {
+    {
         std::vector<int> head(P.fx.radix.begin(), P.fx.radix.end() - 1);
-        if (head.empty()) { h->kx3 = k_xfft_prod_s<3, 4, 1, 1, 1>; h->kx7 = k_xfft_prod_s<7, 4, 1, 1, 1>; h->xspecial = true; }
-#define X(a, b, c) { const int r[3] = {a, b, c}; if (same_list(head, 3, r)) { h->kx3 = k_xfft_prod_s<3, 4, a, b, c>; h->kx7 = k_xfft_prod_s<7, 4, a, b, c>; h->xspecial = true; } }
+        if (head.empty() && F == 4) { h->kx3 = k_xfft_prod_s<3, 4, 1, 1, 1>; h->kx7 = k_xfft_prod_s<7, 4, 1, 1, 1>; h->xspecial = true; }
+        if (head.empty() && F == 8) { h->kx3 = k_xfft_prod_s<3, 8, 1, 1, 1>; h->kx7 = k_xfft_prod_s<7, 8, 1, 1, 1>; h->xspecial = true; }
+#define X(f, a, b, c) { const int r[3] = {a, b, c}; if (F == f && same_list(head, 3, r)) { h->kx3 = k_xfft_prod_s<3, f, a, b, c>; h->kx7 = k_xfft_prod_s<7, f, a, b, c>; h->xspecial = true; } }
         CHAN_XPLANS(X)
 #undef X
     }
@@ -266,7 +268,9 @@ int run_ysolve(chan_t* h) {
     MeanParams M;
     M.ny = P.ny; M.nm = h->nm; M.A2 = h->tab[0][1]; M.B2 = h->tab[0][2]; M.wq = h->wq; M.wm = h->wm; M.wp = h->wp;
     M.nu = P.nu; M.dt = P.dt; M.alpha = Y.alpha; M.beta = Y.beta; M.gamma = Y.gamma; M.zeta = Y.zeta; M.forcing = P.forcing;
-    PB(CHAN_KC_MEAN); k_mean<<<1, 32, 0, h->stream>>>(M, h->H1, h->H3, h->U, h->W, h->H1p, h->H3p, h->meanwork, h->scal); LAUNCHED();
+    const size_t smm = (size_t)15 * P.ny * 8;
+    CK(cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smm));
+    PB(CHAN_KC_MEAN); k_mean<<<1, 256, smm, h->stream>>>(M, h->H1, h->H3, h->U, h->W, h->H1p, h->H3p, h->scal); LAUNCHED();
     const unsigned g = ygrid(h);
     PB(CHAN_KC_Y1); k_y1<<<g, kThreadsY, 0, h->stream>>>(Y, h->H1, h->H3, h->omy, h->hg, h->z1, h->facA, h->facB, h->z2); LAUNCHED();
     PB(CHAN_KC_Y2); k_y2<<<g, kThreadsY, 0, h->stream>>>(Y, h->H2, h->z1, h->z2, h->facA, h->facB, h->phi, h->hv, h->omy, h->z1, h->r1); LAUNCHED();
@@ -314,6 +318,7 @@ int chan_create(chan_t** out, const chan_grid_t* grid, const chan_box_t* box, do
     choose_tiling(h);
     pick_kernels(h);
     if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * 16 > 220 * 1024) { delete h; return CHAN_EINVAL; }
+    if ((size_t)15 * h->P.ny * 8 > 220 * 1024) { delete h; return CHAN_EINVAL; }   // mean-mode solve lives in shared memory
     h->need = carve(h, nullptr);
     *out = h;
     return CHAN_OK;

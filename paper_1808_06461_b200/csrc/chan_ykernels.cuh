@@ -24,6 +24,12 @@ CHAN_HD c2 muli(c2 a) { return mk(-a.y, a.x); }  // i * a
 CHAN_HD c2 ldc(const double2* p) { double2 v = *p; return mk(v.x, v.y); }
 CHAN_HD void stc(double2* p, c2 v) { *p = make_double2(v.x, v.y); }
 
+// L2 prefetch of a row that a marching sweep will read CHAN_PF iterations later: the sweeps are bound by
+// the latency of one dependent global round trip per row, not by bandwidth, at the occupancy their
+// register windows allow.
+#define CHAN_PF 6
+__device__ __forceinline__ void pf2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 struct YTab {               // device pointers to the row tables of one orientation
     const double* B1;       // [ny][8]
     const double* A2;       // [ny][8]
@@ -177,6 +183,7 @@ __global__ void __launch_bounds__(128) k_d1_forward(YParams P, const double2* __
     D1Fwd fw; fw.init();
     double b1[8], lu[8];
     for (int jj = 0; jj < ny + 3; ++jj) {
+        if (jj + CHAN_PF < ny) pf2(f + (size_t)(jj + CHAN_PF) * P.nm + m);
         push(w, jj < ny ? ldc(f + (size_t)jj * P.nm + m) : mk(0, 0));
         const int j = jj - 3;
         if (j >= 0) {
@@ -213,6 +220,7 @@ __global__ void __launch_bounds__(128) k_derive_down(YParams P, const double2* z
     for (int ii = 0; ii < ny + 3; ++ii) {       // ii: virtual (flipped) index of the row being produced
         const int j = ny - 1 - ii;             // physical row
         c2 uj = mk(0, 0), wj = mk(0, 0);
+        if (j - CHAN_PF >= 0) { pf2(zv + (size_t)(j - CHAN_PF) * P.nm + m); pf2(omy + (size_t)(j - CHAN_PF) * P.nm + m); }
         if (ii < ny) {
             load8(P.t[0].lu1, j, lu);
             c2 dv = bs.step(lu, ldc(zv + (size_t)j * P.nm + m));
@@ -312,6 +320,7 @@ __global__ void __launch_bounds__(128) k_y1(YParams P, const double2* H1, const 
     RhsFwd<c2> rz; rz.z1 = rz.z2 = rz.z3 = mk(0, 0);
     double b1[8], lu[8], a2[8], b2[8], a[7];
     for (int jj = 0; jj < ny + 3; ++jj) {
+        if (jj + CHAN_PF < ny) { const size_t op = (size_t)(jj + CHAN_PF) * P.nm + m; pf2(H1 + op); pf2(H3 + op); pf2(omy + op); pf2(hg + op); }
         if (jj < ny) {
             const size_t o = (size_t)jj * P.nm + m;
             c2 h1 = ldc(H1 + o), h3 = ldc(H3 + o), x = ldc(omy + o), gp = ldc(hg + o);
@@ -363,6 +372,10 @@ __global__ void __launch_bounds__(128) k_y2(YParams P, const double2* __restrict
     double lu[8], a2[8], b2[8], a[7];
     for (int ii = 0; ii < ny + 3; ++ii) {
         const int j = ny - 1 - ii;
+        if (j - CHAN_PF >= 0) {
+            const size_t op = (size_t)(j - CHAN_PF) * P.nm + m;
+            pf2(facA + op); pf2(facB + op); pf2(zom + op); pf2(zd + op); pf2(H2 + op); pf2(phi + op); pf2(hv + op);
+        }
         if (ii < ny) {
             const size_t o = (size_t)j * P.nm + m;
             stc(omy + o, bo.step(ld_fac(facA, facB, o), ldc(zom + o)));
@@ -409,6 +422,7 @@ __global__ void __launch_bounds__(128) k_y3(YParams P, double2* facA, double2* f
     RhsFwd<double> ra, rb; ra.z1 = ra.z2 = ra.z3 = 0.0; rb.z1 = rb.z2 = rb.z3 = 0.0;
     double a2[8], b2[8], a[7];
     for (int jj = 0; jj < ny + 3; ++jj) {
+        if (jj + CHAN_PF < ny) { const size_t op = (size_t)(jj + CHAN_PF) * P.nm + m; pf2(facA + op); pf2(facB + op); pf2(zphi + op); pf2(zb + op); }
         if (jj < ny) {
             const size_t o = (size_t)jj * P.nm + m;
             const double4 f = ld_fac(facA, facB, o);
@@ -496,87 +510,87 @@ struct MeanParams {
     double nu, dt, alpha, beta, gamma, zeta;
     int forcing;
 };
-__global__ void k_mean(MeanParams M, const double2* __restrict__ H1, const double2* __restrict__ H3,
-                       double* __restrict__ U, double* __restrict__ W, double* __restrict__ H1p, double* __restrict__ H3p,
-                       double* __restrict__ work /* 8*ny */, double* __restrict__ scal) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+// One CTA; dynamic shared memory 15*ny doubles: the matrix rows and right-hand sides are built by all threads,
+// the (serial) factorisation and substitutions run in thread 0 out of shared memory.
+__global__ void __launch_bounds__(256) k_mean(MeanParams M, const double2* __restrict__ H1, const double2* __restrict__ H3,
+                                              double* __restrict__ U, double* __restrict__ W, double* __restrict__ H1p,
+                                              double* __restrict__ H3p, double* __restrict__ scal) {
+    extern __shared__ double sh[];
     const int ny = M.ny;
+    double* Mt = sh;                  // [ny][8] rows of B2 - c A2 (Dirichlet rows at the walls)
+    double* zu = sh + (size_t)8 * ny; double* zh = zu + ny; double* zw = zh + ny;
+    double* f1 = zw + ny; double* f2 = f1 + ny; double* f3 = f2 + ny; double* fd = f3 + ny;
     const double c = 1.0 / (M.beta * M.nu * M.dt);
-    double* fd = work;            // 1/d
-    double* f1 = work + ny; double* f2 = work + 2 * ny; double* f3 = work + 3 * ny;
-    double* zu = work + 4 * ny; double* zh = work + 5 * ny; double* zw = work + 6 * ny; double* tmp = work + 7 * ny;
-    // explicit parts t = X + dt (gamma H + zeta Hprev)
-    for (int j = 0; j < ny; ++j) {
+    const double g = M.alpha * M.nu * M.dt;
+    // explicit parts t = X + dt (gamma H + zeta Hprev), kept in f1 (U) and f2 (W); old U, W in f3, fd
+    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
         const double h1 = H1[(size_t)j * M.nm].x, h3 = H3[(size_t)j * M.nm].x;
-        zu[j] = U[j] + M.dt * (M.gamma * h1 + M.zeta * H1p[j]);
-        zw[j] = W[j] + M.dt * (M.gamma * h3 + M.zeta * H3p[j]);
+        f1[j] = U[j] + M.dt * (M.gamma * h1 + M.zeta * H1p[j]);
+        f2[j] = W[j] + M.dt * (M.gamma * h3 + M.zeta * H3p[j]);
+        f3[j] = U[j]; fd[j] = W[j];
         H1p[j] = h1; H3p[j] = h3;
     }
-    // right-hand sides into tmp-less form: compute all three before overwriting (need windows of zu,U etc.)
-    // r_u[j] = -c (A2 zu + g B2 U), r_h[j] = -c (A2 1), r_w[j] = -c (A2 zw + g B2 W)
-    const double g = M.alpha * M.nu * M.dt;
-    double* ru = f1; double* rh = f2; double* rw = f3;   // temporarily
-    for (int j = 0; j < ny; ++j) {
-        double su = 0, sh = 0, sw = 0;
-        if (j > 0 && j < ny - 1) {
-            for (int k = 0; k < 7; ++k) {
-                const int jj = j + k - 3;
-                if (jj < 0 || jj >= ny) continue;
-                const double a2 = M.A2[(size_t)j * 8 + k], b2 = M.B2[(size_t)j * 8 + k];
-                su += a2 * zu[jj] + g * b2 * U[jj];
-                sw += a2 * zw[jj] + g * b2 * W[jj];
-                sh += a2;
+    __syncthreads();
+    // r_u = -c (A2 t_u + g B2 U), r_h = -c (A2 1), r_w = -c (A2 t_w + g B2 W); matrix rows
+    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+        double su = 0, sh_ = 0, sw = 0;
+        const bool wall = (j == 0 || j == ny - 1);
+        for (int k = 0; k < 7; ++k) {
+            const double a2 = M.A2[(size_t)j * 8 + k], b2 = M.B2[(size_t)j * 8 + k];
+            Mt[(size_t)j * 8 + k] = wall ? (k == 3 ? 1.0 : 0.0) : b2 - c * a2;
+            const int jj = j + k - 3;
+            if (wall || jj < 0 || jj >= ny) continue;
+            su += a2 * f1[jj] + g * b2 * f3[jj];
+            sw += a2 * f2[jj] + g * b2 * fd[jj];
+            sh_ += a2;
+        }
+        zu[j] = -c * su; zh[j] = -c * sh_; zw[j] = -c * sw;
+        if (wall) { zu[j] = 0.0; zh[j] = 0.0; zw[j] = 0.0; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double d1 = 1, u11 = 0, u12 = 0, u13 = 0, d2 = 1, u21 = 0, u22 = 0, u23 = 0, d3 = 1, u31 = 0, u32 = 0, u33 = 0;
+        double* zs[3] = {zu, zh, zw};
+        for (int j = 0; j < ny; ++j) {
+            double a[7];
+            for (int k = 0; k < 7; ++k) a[k] = Mt[(size_t)j * 8 + k];
+            const double l3 = a[0] * d3; a[1] -= l3 * u31; a[2] -= l3 * u32; a[3] -= l3 * u33;
+            const double l2 = a[1] * d2; a[2] -= l2 * u21; a[3] -= l2 * u22; a[4] -= l2 * u23;
+            const double l1 = a[2] * d1; a[3] -= l1 * u11; a[4] -= l1 * u12; a[5] -= l1 * u13;
+            const double di = 1.0 / a[3];
+            d3 = d2; u31 = u21; u32 = u22; u33 = u23; d2 = d1; u21 = u11; u22 = u12; u23 = u13;
+            d1 = di; u11 = a[4]; u12 = a[5]; u13 = a[6];
+            for (int q = 0; q < 3; ++q) {
+                double z = zs[q][j];
+                if (j >= 3) z -= l3 * zs[q][j - 3];
+                if (j >= 2) z -= l2 * zs[q][j - 2];
+                if (j >= 1) z -= l1 * zs[q][j - 1];
+                zs[q][j] = z;
             }
-            su *= -c; sh *= -c; sw *= -c;
+            fd[j] = di; f1[j] = a[4]; f2[j] = a[5]; f3[j] = a[6];
         }
-        ru[j] = su; rh[j] = sh; rw[j] = sw;
-    }
-    for (int j = 0; j < ny; ++j) { zu[j] = ru[j]; zh[j] = rh[j]; zw[j] = rw[j]; }
-    // factor B2 - c A2 with Dirichlet rows, forward substitute the three right-hand sides
-    double d1 = 1, u11 = 0, u12 = 0, u13 = 0, d2 = 1, u21 = 0, u22 = 0, u23 = 0, d3 = 1, u31 = 0, u32 = 0, u33 = 0;
-    for (int j = 0; j < ny; ++j) {
-        double a[7];
-        for (int k = 0; k < 7; ++k) a[k] = (j == 0 || j == ny - 1) ? (k == 3 ? 1.0 : 0.0) : M.B2[(size_t)j * 8 + k] - c * M.A2[(size_t)j * 8 + k];
-        const double l3 = a[0] * d3; a[1] -= l3 * u31; a[2] -= l3 * u32; a[3] -= l3 * u33;
-        const double l2 = a[1] * d2; a[2] -= l2 * u21; a[3] -= l2 * u22; a[4] -= l2 * u23;
-        const double l1 = a[2] * d1; a[3] -= l1 * u11; a[4] -= l1 * u12; a[5] -= l1 * u13;
-        const double di = 1.0 / a[3];
-        d3 = d2; u31 = u21; u32 = u22; u33 = u23; d2 = d1; u21 = u11; u22 = u12; u23 = u13;
-        d1 = di; u11 = a[4]; u12 = a[5]; u13 = a[6];
-        fd[j] = di; tmp[j] = a[4];
-        // forward substitution (needs previous z's)
-        double* zs[3] = {zu, zh, zw};
-        for (int q = 0; q < 3; ++q) {
-            double z = zs[q][j];
-            if (j >= 3) z -= l3 * zs[q][j - 3];
-            if (j >= 2) z -= l2 * zs[q][j - 2];
-            if (j >= 1) z -= l1 * zs[q][j - 1];
-            zs[q][j] = z;
+        for (int j = ny - 1; j >= 0; --j) {
+            for (int q = 0; q < 3; ++q) {
+                double x = zs[q][j];
+                if (j + 1 < ny) x -= f1[j] * zs[q][j + 1];
+                if (j + 2 < ny) x -= f2[j] * zs[q][j + 2];
+                if (j + 3 < ny) x -= f3[j] * zs[q][j + 3];
+                zs[q][j] = x * fd[j];
+            }
         }
-        f1[j] = a[4]; f2[j] = a[5]; f3[j] = a[6];
-    }
-    for (int j = ny - 1; j >= 0; --j) {
-        double* zs[3] = {zu, zh, zw};
-        for (int q = 0; q < 3; ++q) {
-            double x = zs[q][j];
-            if (j + 1 < ny) x -= f1[j] * zs[q][j + 1];
-            if (j + 2 < ny) x -= f2[j] * zs[q][j + 2];
-            if (j + 3 < ny) x -= f3[j] * zs[q][j + 3];
-            zs[q][j] = x * fd[j];
+        double qp = 0, qh = 0;
+        for (int j = 0; j < ny; ++j) { qp += M.wq[j] * zu[j]; qh += M.wq[j] * zh[j]; }
+        double Pi;
+        if (M.forcing == 0) { Pi = (scal[1] - qp) / qh; scal[0] = Pi / ((M.gamma + M.zeta) * M.dt); }
+        else Pi = scal[0] * (M.gamma + M.zeta) * M.dt;
+        double sm = 0, sp = 0;
+        for (int j = 0; j < ny; ++j) {
+            const double un = zu[j] + Pi * zh[j];
+            U[j] = un; W[j] = zw[j];
+            sm += M.wm[j] * un; sp += M.wp[j] * un;
         }
+        scal[2] = M.nu * sm; scal[3] = -M.nu * sp;
     }
-    double qp = 0, qh = 0;
-    for (int j = 0; j < ny; ++j) { qp += M.wq[j] * zu[j]; qh += M.wq[j] * zh[j]; }
-    double Pi;
-    if (M.forcing == 0) { Pi = (scal[1] - qp) / qh; scal[0] = Pi / ((M.gamma + M.zeta) * M.dt); }
-    else Pi = scal[0] * (M.gamma + M.zeta) * M.dt;
-    double sm = 0, sp = 0;
-    for (int j = 0; j < ny; ++j) {
-        const double un = zu[j] + Pi * zh[j];
-        U[j] = un; W[j] = zw[j];
-        sm += M.wm[j] * un; sp += M.wp[j] * un;
-    }
-    scal[2] = M.nu * sm; scal[3] = -M.nu * sp;
 }
 
 __global__ void k_flux(int ny, const double* __restrict__ wq, const double* __restrict__ U, double* __restrict__ scal) {
