@@ -12,6 +12,7 @@
 #include "chan_fftkernels.cuh"
 #include "chan_plan.h"
 #include "chan_ykernels.cuh"
+#include "chan_ysweeps.cuh"
 
 using namespace chn;
 
@@ -156,13 +157,20 @@ PlaneParams pparams(const chan_t* h) {
 
 inline unsigned ygrid(const chan_t* h) { return (unsigned)((h->nm + kThreadsY - 1) / kThreadsY); }
 
-// a1-a2: state -> u, w, om_x, om_z
+inline unsigned sgrid(const chan_t* h) { return (unsigned)((2 * h->nm + YNT - 1) / YNT); }
+
+// a1-a2, second half: zv (in s1) -> u, w, om_x, om_z
+int run_derive_tail(chan_t* h) {
+    YParams Y = yparams(h);
+    PB(CHAN_KC_DERIVE_DOWN); k_se<<<sgrid(h), YNT, 0, h->stream>>>(Y, h->s1, h->omy, h->U, h->W, h->u, h->w, h->oz); LAUNCHED();
+    PB(CHAN_KC_DERIVE_UP); k_sf<<<sgrid(h), YNT, 0, h->stream>>>(Y, h->s1, h->oz, h->v, h->ox); LAUNCHED();
+    return CHAN_OK;
+}
+// a1-a2 from the state alone
 int run_derive(chan_t* h) {
     YParams Y = yparams(h);
-    PB(CHAN_KC_D1FWD); k_d1_forward<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->v, h->z1); LAUNCHED();
-    PB(CHAN_KC_DERIVE_DOWN); k_derive_down<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->z1, h->omy, h->U, h->W, h->u, h->w, h->s1, h->oz); LAUNCHED();
-    PB(CHAN_KC_DERIVE_UP); k_derive_up<<<ygrid(h), kThreadsY, 0, h->stream>>>(Y, h->s1, h->oz, h->v, h->ox, h->oz); LAUNCHED();
-    return CHAN_OK;
+    PB(CHAN_KC_D1FWD); k_sd0<<<sgrid(h), YNT, 0, h->stream>>>(Y, h->v, h->s1); LAUNCHED();
+    return run_derive_tail(h);
 }
 
 // ---- plan -> kernel dispatch -------------------------------------------------------------------------
@@ -271,13 +279,14 @@ int run_ysolve(chan_t* h) {
     const size_t smm = (size_t)15 * P.ny * 8;
     CK(cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smm));
     PB(CHAN_KC_MEAN); k_mean<<<1, 256, smm, h->stream>>>(M, h->H1, h->H3, h->U, h->W, h->H1p, h->H3p, h->scal); LAUNCHED();
-    const unsigned g = ygrid(h);
-    PB(CHAN_KC_Y1); k_y1<<<g, kThreadsY, 0, h->stream>>>(Y, h->H1, h->H3, h->omy, h->hg, h->z1, h->facA, h->facB, h->z2); LAUNCHED();
-    PB(CHAN_KC_Y2); k_y2<<<g, kThreadsY, 0, h->stream>>>(Y, h->H2, h->z1, h->z2, h->facA, h->facB, h->phi, h->hv, h->omy, h->z1, h->r1); LAUNCHED();
-    PB(CHAN_KC_Y3); k_y3<<<g, kThreadsY, 0, h->stream>>>(Y, h->facA, h->facB, h->z1, h->r1, h->r2, h->z2, h->r3, h->r4); LAUNCHED();
-    PB(CHAN_KC_Y4); k_y4<<<g, kThreadsY, 0, h->stream>>>(Y, h->facA, h->facB, h->z2, h->r3, h->r4, h->coef); LAUNCHED();
-    dim3 g5(g, P.ny < 64 ? P.ny : 64);
-    PB(CHAN_KC_Y5); k_y5<<<g5, kThreadsY, 0, h->stream>>>(Y, h->coef, h->z1, h->r2, h->r1, h->z2, h->r3, h->r4, h->phi, h->v); LAUNCHED();
+    // buffers that are dead during the y-phase carry its scratch:
+    // s1: zd -> z_phi -> phi_p -> zv;  oz: R_om -> z_om -> z_vab;  u, ox: factor rows (H1, H3 are consumed by SA);
+    // w: z_vp (H2 is consumed by SB);  v: phi_ab, then the new v in place
+    const unsigned g = sgrid(h);
+    PB(CHAN_KC_Y1); k_sa<<<g, YNT, 0, h->stream>>>(Y, h->H1, h->H3, h->omy, h->hg, h->s1, h->oz); LAUNCHED();
+    PB(CHAN_KC_Y2); k_sb<<<g, YNT, 0, h->stream>>>(Y, h->H2, h->phi, h->hv, h->s1, h->oz, h->u, h->ox); LAUNCHED();
+    PB(CHAN_KC_Y3); k_sc<<<g, YNT, 0, h->stream>>>(Y, h->u, h->ox, h->oz, h->s1, h->omy, h->v, h->w, h->coef); LAUNCHED();
+    PB(CHAN_KC_Y4); k_sd<<<g, YNT, 0, h->stream>>>(Y, h->u, h->ox, h->w, h->oz, h->s1, h->v, h->coef, h->phi); LAUNCHED();
     return CHAN_OK;
 }
 
@@ -426,7 +435,7 @@ int chan_substep(chan_t* h) {
     if ((rc = run_nonlinear(h))) return rc;
     if ((rc = run_ysolve(h))) return rc;
     h->isub = (h->isub + 1) % 3;
-    return run_derive(h);
+    return run_derive_tail(h);
 }
 
 int chan_step(chan_t* h) {
