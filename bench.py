@@ -36,7 +36,7 @@ UNIT = "Mpoint*substeps/s"
 # one complex field pass = 8 B/point).  The SURVEY groups are the section 8(d) figures.
 BYTES_PER_POINT = {
     "d1_forward": 16, "derive_down": 48, "derive_up": 40, "zfft_inv": 120, "xfft_prod": 108, "zfft_fwd": 60,
-    "y1": 72, "y2": 100, "y3": 76, "y4": 48, "y5": 48, "stats": 48, "transpose": 16,
+    "y1": 56, "y2": 80, "y3": 88, "y4": 72, "stats": 48, "transpose": 16,   # y1..y4 = sweeps SA..SD, derive_* = SE, SF
 }
 SURVEY_GROUPS = {
     "K2 z-pad + inverse z-FFT": (["zfft_inv"], 120),
