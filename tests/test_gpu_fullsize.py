@@ -1,0 +1,206 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (same plans, tiles, chunking).
+
+The oracle cannot run a 768x251x576 (or larger) substep in seconds, but every stage of the path is separable:
+the wall-normal stages act on each (kx,kz) line independently and the wall-parallel stages on each y-plane
+independently.  So the full-size GPU result is compared with the oracle on SAMPLED lines and planes:
+
+* lines: a small ChannelOracle on the same mesh whose wavenumber tables are overwritten with those of a
+  sub-lattice {p} x {z slot} of the big grid (including the mean mode and the z-Nyquist slot) computes exactly
+  those lines of the big problem;
+* planes: a ChannelOracle with the full nx, nz but only the sampled planes runs the padded transforms, the
+  products, the filter products and the statistics of those planes.
+
+All inputs are seeded; the oracle receives copies of the very arrays handed to the library.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import __graft_entry__ as entry
+from oracle.channel import ChannelOracle
+from paper_1808_06461_b200 import inputs
+from test_gpu_parity import TwinOracle, rel
+
+pytestmark = pytest.mark.gpu
+
+TOL_SUBSTEP = 1e-11
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    entry.build()
+    from paper_1808_06461_b200 import binding
+    return binding
+
+
+def sub_lattice(c, npx=8, nsz=8):
+    """Index lists (p, z slot) of the sampled lines; entry [0] of each is 0 (mean mode) and the middle z entry is
+    the Nyquist slot, so the small oracle's special cases coincide with the big grid's."""
+    nxh, nz = c["nx"] // 2, c["nz"]
+    rng = np.random.default_rng(11)
+    ps = np.sort(np.concatenate([[0, 1, nxh - 1], rng.choice(np.arange(2, nxh - 1), npx - 3, replace=False)]))
+    lo = np.sort(np.concatenate([[0, 1], rng.choice(np.arange(2, nz // 2), nsz // 2 - 2, replace=False)]))
+    hi = np.sort(np.concatenate([[nz - 1], rng.choice(np.arange(nz // 2 + 1, nz - 1), nsz // 2 - 2, replace=False)]))
+    ss = np.concatenate([lo, [nz // 2], hi])
+    assert ps.size == npx and ss.size == nsz and ss[nsz // 2] == nz // 2
+    return ps, ss
+
+
+def line_oracle(c, ps, ss, cls=ChannelOracle):
+    from oracle.channel import wavenumbers
+    kx, kz, _ = wavenumbers(c["nx"], c["nz"], c["lx"], c["lz"])
+    o = cls(2 * ps.size, c["ny"], ss.size, c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    o.kx, o.kz = kx[ps].copy(), kz[ss].copy()
+    o.k2 = o.kz[:, None] ** 2 + o.kx[None, :] ** 2
+    return o
+
+
+def take_lines(t, ps, ss):
+    """[nz][nxh][ny] torch tensor (any device) -> numpy [len(ss)][len(ps)][ny]."""
+    idx_s = torch.as_tensor(ss, device=t.device)
+    idx_p = torch.as_tensor(ps, device=t.device)
+    return t.index_select(0, idx_s).index_select(1, idx_p).cpu().numpy()
+
+
+def random_field(shape, nz, seed, dev, scale=1.0):
+    g = torch.Generator(device=dev).manual_seed(seed)
+    f = torch.view_as_complex(torch.randn(shape + (2,), generator=g, dtype=torch.float64, device=dev)) * scale
+    q = torch.arange(1, nz // 2, device=dev)
+    f[nz - q, 0] = torch.conj(f[q, 0])          # Hermitian p = 0 column
+    f[0, 0] = f[0, 0].real + 0j
+    f[nz // 2] = 0
+    return f
+
+
+def fullsize_names():
+    names = ["cfg3"]
+    if os.environ.get("CHAN_TEST_CFG4", "0") == "1":
+        names.append("cfg4")
+    return names
+
+
+@pytest.mark.parametrize("name", fullsize_names())
+def test_fullsize_planes_filter_stats(B, name):
+    """a3-a8, a13, a14 at full size on sampled planes, from six seeded random Hermitian fields."""
+    c = inputs.config(name)
+    dev = torch.device("cuda:0")
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
+    nz, ny = c["nz"], c["ny"]
+    planes = [0, 1, 2, ny // 3, ny // 2, 2 * ny // 3, ny - 2, ny - 1]    # the oracle wants at least 8 mesh points
+    fids = (B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ)
+    z = torch.zeros(ch.shape, dtype=torch.complex128, device=dev)
+    ch.set_state(z, z, z, c["U"], c["W"])       # the filter and the statistics want a state; the six fields are overwritten below
+    ch._keep = None
+    del z
+    sampled = []
+    for k, fid in enumerate(fids):
+        f = random_field(ch.shape, nz, 1000 + k, dev)
+        ch.debug_set_field(fid, f)
+        sampled.append(f[:, :, planes].cpu().numpy())
+        del f
+    torch.cuda.empty_cache()
+    o = ChannelOracle(c["nx"], len(planes), nz, c["lx"], c["lz"], np.linspace(-1, 1, len(planes)), c["re"], c["dt"])
+    # filter (a13): bit-exact mode selection, products on the dealiased grid
+    kxc, kzc = c["cut"]
+    got = ch.filter_store(kxc, kzc)
+    gp = got[:, planes].cpu().numpy()
+    del got
+    slots = [q % nz for q in list(range(0, kzc + 1)) + list(range(-kzc, 0))]
+    for n in range(3):
+        assert np.array_equal(gp[n], np.transpose(sampled[n][slots][:, : kxc + 1, :], (2, 0, 1))), n
+    pu, pv, pw, pox, poy, poz = (o.to_physical(f) for f in sampled)
+    prods = (pu * pu, pu * pv, pu * pw, pv * pv, pv * pw, pw * pw, pox * pox + poy * poy + poz * poz)
+    for n, pr in enumerate(prods):
+        assert rel(gp[3 + n], o.to_spectral(pr, kxc, kzc)) < 1e-13, n
+    # statistics (a14)
+    ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
+    prof, ns = ch.stats(B.STATS_READ)
+    assert ns == 1
+    wp = np.full(c["nx"] // 2, 2.0)
+    wp[0] = 1.0
+    mean = lambda a, b: np.einsum("p,qpy->y", wp, (a * np.conj(b)).real)
+    u, v, w, ox, oy, oz = sampled
+    ref = [u[0, 0].real, v[0, 0].real, w[0, 0].real, mean(u, u), mean(u, v), mean(u, w), mean(v, v), mean(v, w), mean(w, w),
+           mean(ox, ox) + mean(oy, oy) + mean(oz, oz)]
+    for n in range(10):
+        assert np.abs(prof[n][planes] - ref[n]).max() < 1e-12 * max(1.0, np.abs(ref[n]).max()), n
+    # second-order consistency on the GPU side: (0,0) mode of the stored products == plane statistics
+    for n in range(3, 10):
+        assert np.abs(gp[n][:, 0, 0].real - prof[n][planes]).max() < 1e-11 * np.abs(prof[n]).max()
+    # nonlinear term (a3-a8)
+    ch.debug_run_stage(B.STAGE_NONLINEAR)
+    H = o.nonlinear(sampled)
+    for fid, ref_h in zip((B.F_H1, B.F_H2, B.F_H3), H):
+        g = ch.debug_get_field(fid)
+        assert rel(g[:, :, planes], ref_h) < 1e-13, fid
+        assert not bool(g[nz // 2].any())
+        del g
+    ch.close()
+
+
+@pytest.mark.parametrize("name", fullsize_names())
+def test_fullsize_lines_derive_and_ysolve(B, name):
+    """a1-a2 and a9-a12 at full size on a sub-lattice of lines, for the three substep coefficient sets."""
+    c = inputs.config(name)
+    dev = torch.device("cuda:0")
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
+    nz = c["nz"]
+    ps, ss = sub_lattice(c)
+    v, phi, omy = inputs.fluctuations(c, device=dev, zchunk=64)
+    sv, sphi, somy = (take_lines(t, ps, ss) for t in (v, phi, omy))
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    del v, phi, omy
+    ch._keep = None
+    torch.cuda.empty_cache()
+    o = line_oracle(c, ps, ss)
+    o.set_state(sv, sphi, somy, c["U"], c["W"])
+    # a1-a2
+    refs = o.velocities_vorticities()
+    for fid, ref in zip((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ), refs):
+        g = ch.debug_get_field(fid)
+        assert rel(take_lines(g, ps, ss), ref) < 1e-12, fid
+        del g
+    # a9-a12 with seeded H and history
+    Hs, Hl = [], []
+    for k, fid in enumerate((B.F_H1, B.F_H2, B.F_H3, B.F_HV_PREV, B.F_HG_PREV)):
+        f = random_field(ch.shape, nz, 2000 + k, dev, scale=1e2 if k < 3 else 1.0)
+        if k >= 3:
+            f[0, 0] = 0
+        Hl.append(take_lines(f, ps, ss))
+        Hs.append(f)
+    for isub in range(3):
+        o, t = line_oracle(c, ps, ss), line_oracle(c, ps, ss, TwinOracle)     # fresh: no mean-flow history
+        for orc in (o, t):
+            orc.set_state(sv, sphi, somy, c["U"], c["W"])
+            orc.isub = isub
+            orc.hv_prev, orc.hg_prev = Hl[3].copy(), Hl[4].copy()
+            orc.nonlinear = lambda fields: tuple(h.copy() for h in Hl[:3])
+            orc.substep()
+        v, phi, omy = inputs.fluctuations(c, device=dev, zchunk=64)
+        ch.set_state(v, phi, omy, c["U"], c["W"])
+        del v, phi, omy
+        ch._keep = None
+        for f, fid in zip(Hs, (B.F_H1, B.F_H2, B.F_H3, B.F_HV_PREV, B.F_HG_PREV)):
+            ch.debug_set_field(fid, f)
+        ch.debug_set_substep_index(isub)
+        ch.debug_run_stage(B.STAGE_YSOLVE)
+        gv, gphi, gomy, gU, gW = ch.get_state()
+        e = {"v": rel(take_lines(gv, ps, ss), o.v), "phi": rel(take_lines(gphi, ps, ss), o.phi),
+             "omy": rel(take_lines(gomy, ps, ss), o.omy), "U": rel(gU, o.U)}
+        fl = {"v": rel(t.v, o.v), "phi": rel(t.phi, o.phi), "omy": rel(t.omy, o.omy), "U": rel(t.U, o.U)}
+        del gv, gphi, gomy
+        print(f"{name} substep {isub}: |gpu-oracle| {e}  |twin-oracle| {fl}")
+        for k in e:
+            assert e[k] < max(TOL_SUBSTEP, 2.0 * fl[k]), (isub, k, e, fl)
+        assert rel(take_lines(ch.debug_get_field(B.F_HV_PREV), ps, ss), o.hv_prev) < 1e-11
+        assert rel(take_lines(ch.debug_get_field(B.F_HG_PREV), ps, ss), o.hg_prev) < 1e-13
+        # the new state's derived fields (a1 chained behind the y-solve) on the same lines
+        ch.debug_run_stage(B.STAGE_DERIVE)
+        refs = o.velocities_vorticities()
+        for fid, ref in zip((B.F_U, B.F_W, B.F_OMX, B.F_OMZ), (refs[0], refs[2], refs[3], refs[5])):
+            assert rel(take_lines(ch.debug_get_field(fid), ps, ss), ref) < 1e-8, fid
+    ch.close()
