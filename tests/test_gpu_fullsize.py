@@ -12,6 +12,7 @@ independently.  So the full-size GPU result is compared with the oracle on SAMPL
 
 All inputs are seeded; the oracle receives copies of the very arrays handed to the library.
 """
+import copy
 import os
 
 import numpy as np
@@ -85,14 +86,15 @@ def fullsize_names():
     return env.split(",") if env else ["cfg3", "cfg4"]
 
 
-@pytest.mark.parametrize("name", fullsize_names())
+@pytest.mark.parametrize("name", fullsize_names() + ["cfg5-planes"])
 def test_fullsize_planes_filter_stats(B, name):
-    """a3-a8, a13, a14 at full size on sampled planes, from six seeded random Hermitian fields."""
-    c = inputs.config(name)
+    """a3-a8, a13, a14 at full size on sampled planes, from six seeded random Hermitian fields.
+    "cfg5-planes": the 1536 x 1152 wall-parallel grid of config 5 (its transform plans and tiles) on 9 planes."""
+    c = inputs.config("cfg5", ny=9) if name == "cfg5-planes" else inputs.config(name)
     dev = torch.device("cuda:0")
     ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
     nz, ny = c["nz"], c["ny"]
-    planes = [0, 1, 2, ny // 3, ny // 2, 2 * ny // 3, ny - 2, ny - 1]    # the oracle wants at least 8 mesh points
+    planes = sorted({0, 1, 2, ny // 3, ny // 2, 2 * ny // 3, ny - 3, ny - 2, ny - 1})    # the oracle wants at least 8 mesh points
     fids = (B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ)
     z = torch.zeros(ch.shape, dtype=torch.complex128, device=dev)
     ch.set_state(z, z, z, c["U"], c["W"])       # the filter and the statistics want a state; the six fields are overwritten below
@@ -144,10 +146,16 @@ def test_fullsize_planes_filter_stats(B, name):
     ch.close()
 
 
-@pytest.mark.parametrize("name", fullsize_names())
+@pytest.mark.parametrize("name", fullsize_names() + ["cfg5-lines"])
 def test_fullsize_lines_derive_and_ysolve(B, name):
-    """a1-a2 and a9-a12 at full size on a sub-lattice of lines, for the three substep coefficient sets."""
-    c = inputs.config(name)
+    """a1-a2 and a9-a12 at full size on a sub-lattice of lines, for the three substep coefficient sets.
+    "cfg5-lines": the 1025-point mesh, Re and dt of config 5 on a 32 x 16 sub-box with the same dx, dz (the same
+    range of wavenumbers and Helmholtz parameters, the full line length)."""
+    if name == "cfg5-lines":
+        c5 = inputs.CONFIGS["cfg5"]
+        c = inputs.config("cfg5", nx=32, nz=16, lx=c5["lx"] * 32 / c5["nx"], lz=c5["lz"] * 16 / c5["nz"])
+    else:
+        c = inputs.config(name)
     dev = torch.device("cuda:0")
     ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
     nz = c["nz"]
@@ -158,7 +166,8 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
     del v, phi, omy
     ch._keep = None
     torch.cuda.empty_cache()
-    o = line_oracle(c, ps, ss)
+    base = line_oracle(c, ps, ss)
+    o = copy.deepcopy(base)
     o.set_state(sv, sphi, somy, c["U"], c["W"])
     # a1-a2
     refs = o.velocities_vorticities()
@@ -175,7 +184,8 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
         Hl.append(take_lines(f, ps, ss))
         Hs.append(f)
     for isub in range(3):
-        o, t = line_oracle(c, ps, ss), line_oracle(c, ps, ss, TwinOracle)     # fresh: no mean-flow history
+        o, t = copy.deepcopy(base), copy.deepcopy(base)     # fresh: no mean-flow history (the exact-rational tables are built once)
+        t.__class__ = TwinOracle
         for orc in (o, t):
             orc.set_state(sv, sphi, somy, c["U"], c["W"])
             orc.isub = isub
