@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -39,6 +40,7 @@ struct chan {
     int pc = 1;            // planes per FFT chunk
     int Tz = 1;            // k_x columns per z-FFT tile
     int xthreads = 128;    // threads per row CTA of the x pass
+    int zthreads = 256;    // threads per tile CTA of the z passes
     void (*kzinv)(PlaneParams, FieldPtrs, int, int, double2*, int) = nullptr;
     void (*kzfwd)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int) = nullptr;
     void (*kx3)(PlaneParams, const double2*, int, double2*, int) = nullptr;
@@ -78,6 +80,9 @@ void choose_tiling(chan_t* h) {
     while (T > 1 && T > P.nxh) T >>= 1;
     h->Tz = T;
     h->xthreads = ((size_t)3 * P.mx * 16 > 72 * 1024) ? 256 : 128;   // <= 3 CTAs per SM: use wider CTAs
+    if (const char* e = std::getenv("CHAN_TZ")) { const int v = std::atoi(e); if (v == 1 || v == 2 || v == 4 || v == 8 || v == 16) h->Tz = v; }
+    if (const char* e = std::getenv("CHAN_ZTHREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 256) h->zthreads = v; }
+    if (const char* e = std::getenv("CHAN_XTHREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 256) h->xthreads = v; }
     const size_t per_plane = (size_t)13 * P.mz * P.nxh * 16;
     long long pc = (long long)(1536ull * 1024 * 1024 / per_plane);
     if (pc < 1) pc = 1;
@@ -182,7 +187,7 @@ int run_derive(chan_t* h) {
     X(6, 8, 8, 4) X(6, 6, 8, 8) X(6, 8, 8, 8)
 #define CHAN_XPLANS(X) X(4, 6, 1, 1) X(4, 12, 1, 1) X(4, 6, 4, 1) X(4, 6, 6, 1) X(4, 6, 8, 1) X(4, 12, 8, 1) X(4, 6, 6, 4) X(4, 6, 6, 6) \
     X(4, 6, 8, 4) X(4, 6, 6, 8) X(4, 6, 8, 8) X(4, 12, 6, 6) X(4, 12, 6, 8) X(4, 12, 8, 8) X(8, 6, 1, 1) X(8, 12, 1, 1) X(8, 12, 6, 1) \
-    X(8, 12, 12, 1) X(8, 6, 8, 1)
+    X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
 
 typedef void (*zinv_fn)(PlaneParams, FieldPtrs, int, int, double2*, int);
 typedef void (*zfwd_fn)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int);
@@ -221,7 +226,7 @@ int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, i
     const size_t sm = (size_t)Q.mz * T * 16;
     CK(cudaFuncSetAttribute((const void*)h->kzinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     dim3 g((Q.nxh + T - 1) / T, npl, nf);
-    PB(CHAN_KC_ZFFT_INV); h->kzinv<<<g, 256, sm, h->stream>>>(Q, in, j0, npl, h->zpad, T); LAUNCHED();
+    PB(CHAN_KC_ZFFT_INV); h->kzinv<<<g, h->zthreads, sm, h->stream>>>(Q, in, j0, npl, h->zpad, T); LAUNCHED();
     return CHAN_OK;
 }
 int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out, double scale, int filt, int kxc, int kzc) {
@@ -230,7 +235,7 @@ int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, cons
     CK(cudaFuncSetAttribute((const void*)h->kzfwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     dim3 g((pin + T - 1) / T, npl, nf);
     PB(filt ? CHAN_KC_ZFFT_FWD_FILTER : CHAN_KC_ZFFT_FWD);
-    h->kzfwd<<<g, 256, sm, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc, T); LAUNCHED();
+    h->kzfwd<<<g, h->zthreads, sm, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc, T); LAUNCHED();
     return CHAN_OK;
 }
 int xprod(chan_t* h, const PlaneParams& Q, int nprod, int npl, int pout) {

@@ -152,12 +152,15 @@ struct FieldPtrsW { double2* f[8]; };
 // column t), t fastest over the lanes: every shared access of 8 lanes is one contiguous 128-byte row and
 // the twiddle of a butterfly is a broadcast load.
 // =====================================================================================================
-template <int R, bool INV, bool DIT, class Src, class Dst>
+// M > 0: the sub-block length as a compile-time constant (specialised kernels), M = 0: taken from the stage.
+template <int R, bool INV, bool DIT, int M = 0, class Src, class Dst>
 CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int T, int tid, int nt) {
-    const int m = S.m, ncur = R * m, nb = n / R;
+    const int m = M > 0 ? M : S.m, ncur = R * m, nb = n / R;
     const int total = nb * T;
+    int lgT = 0;
+    while ((1 << lgT) < T) ++lgT;               // T is a power of two
     for (int w = tid; w < total; w += nt) {
-        const int b = w / T, t = w - b * T;     // T is a power of two
+        const int b = w >> lgT, t = w & (T - 1);
         const int blk = b / m, p = b - blk * m;
         c2 tw[R - 1 > 0 ? R - 1 : 1];
         if (m > 1) {
@@ -304,23 +307,24 @@ __global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
     const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
     ZInvIO io = make_zinv_io(P, T, reinterpret_cast<c2*>(smem_raw), in.f[fi] + (size_t)(j0 + jc) * P.nm,
                              zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
-    const int tid = threadIdx.x, nt = blockDim.x, mz = P.mz;
+    constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
+    const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true; io.gout = (NS == 1);
-    zpass<R0, true, false>(io, io, P.fz.st[0], mz, T, tid, nt);
+    zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
     if constexpr (NS > 1) {
         __syncthreads();
         io.gin = false; io.gout = (NS == 2);
-        zpass<R1, true, false>(io, io, P.fz.st[1], mz, T, tid, nt);
+        zpass<R1, true, false, M1>(io, io, P.fz.st[1], mz, T, tid, nt);
     }
     if constexpr (NS > 2) {
         __syncthreads();
         io.gout = (NS == 3);
-        zpass<R2, true, false>(io, io, P.fz.st[2], mz, T, tid, nt);
+        zpass<R2, true, false, M2>(io, io, P.fz.st[2], mz, T, tid, nt);
     }
     if constexpr (NS > 3) {
         __syncthreads();
         io.gout = true;
-        zpass<R3, true, false>(io, io, P.fz.st[3], mz, T, tid, nt);
+        zpass<R3, true, false, 1>(io, io, P.fz.st[3], mz, T, tid, nt);
     }
 }
 template <int R0, int R1, int R2, int R3>
@@ -332,25 +336,26 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
     ZFwdIO io = make_zfwd_io(P, T, reinterpret_cast<c2*>(smem_raw), xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin,
                              filt ? out.f[fi] + (size_t)j * (2 * kzc + 1) * (kxc + 1) : out.f[fi] + (size_t)j * P.nm, pin, p0, scale,
                              filt, kxc, kzc);
-    const int tid = threadIdx.x, nt = blockDim.x, mz = P.mz;
+    constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
+    const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true;
     if constexpr (NS > 3) {
-        zpass<R3, false, true>(io, io, P.fz.st[3], mz, T, tid, nt);
+        zpass<R3, false, true, 1>(io, io, P.fz.st[3], mz, T, tid, nt);
         __syncthreads();
         io.gin = false;
     }
     if constexpr (NS > 2) {
-        zpass<R2, false, true>(io, io, P.fz.st[2], mz, T, tid, nt);
+        zpass<R2, false, true, M2>(io, io, P.fz.st[2], mz, T, tid, nt);
         __syncthreads();
         io.gin = false;
     }
     if constexpr (NS > 1) {
-        zpass<R1, false, true>(io, io, P.fz.st[1], mz, T, tid, nt);
+        zpass<R1, false, true, M1>(io, io, P.fz.st[1], mz, T, tid, nt);
         __syncthreads();
         io.gin = false;
     }
     io.gout = true;
-    zpass<R0, false, true>(io, io, P.fz.st[0], mz, T, tid, nt);
+    zpass<R0, false, true, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
 }
 #endif
 
@@ -370,9 +375,9 @@ struct XIO {
     CHAN_HD c2 load(int e, int q) const { return sm[q * stride + swz(e)]; }
     CHAN_HD void store(int e, int q, c2 v) const { sm[q * stride + swz(e)] = v; }
 };
-template <int R, bool INV, bool DIT>
+template <int R, bool INV, bool DIT, int M = 0>
 CHAN_HD void xpass(const XIO& io, const FftStage& S, int n, int nseq, int tid, int nt) {
-    const int m = S.m, ncur = R * m, nb = n / R;
+    const int m = M > 0 ? M : S.m, ncur = R * m, nb = n / R;
     for (int b = tid; b < nb; b += nt) {
         const int blk = b / m, p = b - blk * m;
         c2 tw[R - 1];
@@ -517,18 +522,19 @@ __global__ void __launch_bounds__(256, 2) k_xfft_prod_s(CHAN_XARGS) {
     extern __shared__ double2 smem_raw[];
     constexpr int NC = (NPROD + 1) / 2;
     const int r = blockIdx.x, jc = blockIdx.y;
-    const int tid = threadIdx.x, nt = blockDim.x, mx = P.mx;
+    constexpr int M2 = F, M1 = R2 * F, M0 = R1 * R2 * F, mx = R0 * M0;
+    const int tid = threadIdx.x, nt = blockDim.x;
     XIO io; io.sm = reinterpret_cast<c2*>(smem_raw); io.stride = mx;
     xpack(io, mx, P.nxh, zpad + ((size_t)jc * P.mz + r) * P.nxh, (size_t)npl * P.mz * P.nxh, tid, nt);
     __syncthreads();
-    if constexpr (R0 > 1) { xpass<R0, true, false>(io, P.fx.st[0], mx, 3, tid, nt); __syncthreads(); }
-    if constexpr (R1 > 1) { xpass<R1, true, false>(io, P.fx.st[1], mx, 3, tid, nt); __syncthreads(); }
-    if constexpr (R2 > 1) { xpass<R2, true, false>(io, P.fx.st[2], mx, 3, tid, nt); __syncthreads(); }
+    if constexpr (R0 > 1) { xpass<R0, true, false, M0>(io, P.fx.st[0], mx, 3, tid, nt); __syncthreads(); }
+    if constexpr (R1 > 1) { xpass<R1, true, false, M1>(io, P.fx.st[1], mx, 3, tid, nt); __syncthreads(); }
+    if constexpr (R2 > 1) { xpass<R2, true, false, M2>(io, P.fx.st[2], mx, 3, tid, nt); __syncthreads(); }
     xfused<F, NPROD>(io, mx, tid, nt);
     __syncthreads();
-    if constexpr (R2 > 1) { xpass<R2, false, true>(io, P.fx.st[2], mx, NC, tid, nt); __syncthreads(); }
-    if constexpr (R1 > 1) { xpass<R1, false, true>(io, P.fx.st[1], mx, NC, tid, nt); __syncthreads(); }
-    if constexpr (R0 > 1) { xpass<R0, false, true>(io, P.fx.st[0], mx, NC, tid, nt); __syncthreads(); }
+    if constexpr (R2 > 1) { xpass<R2, false, true, M2>(io, P.fx.st[2], mx, NC, tid, nt); __syncthreads(); }
+    if constexpr (R1 > 1) { xpass<R1, false, true, M1>(io, P.fx.st[1], mx, NC, tid, nt); __syncthreads(); }
+    if constexpr (R0 > 1) { xpass<R0, false, true, M0>(io, P.fx.st[0], mx, NC, tid, nt); __syncthreads(); }
     xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
 }
 #endif

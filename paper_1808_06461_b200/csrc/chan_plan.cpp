@@ -253,9 +253,15 @@ int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const doub
     const int maxr = (er && std::atoi(er) >= 2) ? std::atoi(er) : 12;
     int fuse = 4;
     if (ef) fuse = (std::atoi(ef) == 8) ? 8 : 4;
-    else {   // the fused radix (4 or 8) that gives the shorter stage list; 4 on a tie (lighter on registers)
+    else {   // the fused radix (4 or 8) that gives the shorter stage list, then the one without radix-12 stages
+             // (they spill under the 128-register cap), then 4 (lighter fused stage)
         FftPlan f4, f8;
-        if (make_fft_plan(P.mx, 4, maxr, f4) && make_fft_plan(P.mx, 8, maxr, f8) && f8.radix.size() < f4.radix.size()) fuse = 8;
+        auto key = [](const FftPlan& f) {
+            int c12 = 0;
+            for (int r : f.radix) c12 += (r == 12);
+            return (int)f.radix.size() * 100 + c12;
+        };
+        if (make_fft_plan(P.mx, 4, maxr, f4) && make_fft_plan(P.mx, 8, maxr, f8) && key(f8) < key(f4)) fuse = 8;
     }
     if (!make_fft_plan(P.mx, fuse, maxr, P.fx) || !make_fft_plan(P.mz, 0, maxr, P.fz)) return CHAN_EINVAL;
 
