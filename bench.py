@@ -92,6 +92,23 @@ class ClockSampler:
                 "power_w_max": max(float(r[2]) for r in self.rows), "reasons": reasons}
 
 
+def max_over_ranks(ms, world, device):
+    """Device-timed milliseconds of this rank -> the maximum over all ranks (the job's time).  `device` is where the
+    backend wants its tensors (cuda for NCCL, cpu for gloo in the CPU tests)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(npts, substeps, world, ms_max):
+    """Whole-job Mpoint*substeps/s of `world` replicas that each advanced npts points by `substeps` substeps."""
+    return world * npts * substeps / (ms_max * 1e-3) / 1e6
+
+
 def pick_workload(name, free_bytes):
     from paper_1808_06461_b200 import inputs
     if name != "auto":
@@ -137,7 +154,15 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    wl = args.workload if args.workload != "auto" else "cfg4"
+    wl = args.workload
+    if wl == "auto":        # the workload the GPU arm picks on this box (cfg5 on a 180 GB B200)
+        wl = "cfg5"
+        try:
+            import torch
+            if torch.cuda.is_available():
+                wl = pick_workload("auto", torch.cuda.mem_get_info(0)[0])
+        except Exception:
+            pass
     steps = max(1, min(args.steps, 3))
     val, ms, sample = oracle_sample(wl, steps, min(args.warmup, 1))
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
@@ -235,11 +260,8 @@ def main():
     ms_total = e0.elapsed_time(e1)
     prof = ch.debug_profile_read()
     launches = ch.debug_launch_count() - l0
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total_max = float(tmax.item())
-    value = world * 3 * npts * K / (ms_total_max * 1e-3) / 1e6
+    ms_total_max = max_over_ranks(ms_total, world, dev)
+    value = job_value(npts, 3 * K, world, ms_total_max)
     # finite-state check: a blown-up field would make the timing meaningless (the ten filtered variables
     # are linear and quadratic in every velocity and vorticity component)
     finite = bool(torch.isfinite(torch.view_as_real(fout)).all().item())
@@ -314,12 +336,10 @@ def main():
             barrier()
             wall = (time.perf_counter() - t0) * 1e3
             ms_e = max(e0.elapsed_time(e1), wall)       # host-side copies block: take the larger clock
-            te = torch.tensor([ms_e], dtype=torch.float64, device=dev)
-            if world > 1:
-                dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            ms_e = max_over_ranks(ms_e, world, dev)
             state_b = 3 * F + 2 * c["ny"] * 8
-            e2e = {"value": world * 3 * npts * Ke / (float(te.item()) * 1e-3) / 1e6, "unit": UNIT, "steps": Ke,
-                   "ms_per_step": float(te.item()) / Ke, "h2d_bytes_per_step": state_b,
+            e2e = {"value": job_value(npts, 3 * Ke, world, ms_e), "unit": UNIT, "steps": Ke,
+                   "ms_per_step": ms_e / Ke, "h2d_bytes_per_step": state_b,
                    "d2h_bytes_per_step": state_b + hf.numel() * 16 + 10 * c["ny"] * 8,
                    "api": "chan_set_state_host + chan_step + chan_filter_store_host + chan_stats(READ) + chan_get_state_host, "
                           + ("pinned" if pinned else "pageable (pinning refused)") + " host buffers"}
