@@ -65,6 +65,10 @@ CONFIGS = {
                  mean=("reichardt", 2000.0), spec="vk", M=8, amp=("rms", 1.0), cut=(62, 62), seed=4),
     "cfg5": dict(nx=1536, ny=1025, nz=1152, lx=0.8 * math.pi, lz=0.3 * math.pi, re=5300.0, dt=1e-5,
                  mesh=("tanh", 3.0), mean=("reichardt", 5300.0), spec="vk", M=8, amp=("rms", 1.0), cut=(95, 71), seed=5),
+    # config 5 on a 129-plane slab: the same planes, transform plans, tiles and chunks as cfg5 in 1/8 of the memory
+    # (ncu --set full backs the device memory up on the host, which the 146 GB workspace of cfg5 does not survive)
+    "cfg5slab": dict(nx=1536, ny=129, nz=1152, lx=0.8 * math.pi, lz=0.3 * math.pi, re=5300.0, dt=1e-5,
+                     mesh=("tanh", 2.5), mean=("reichardt", 5300.0), spec="vk", M=8, amp=("rms", 1.0), cut=(95, 71), seed=5),
     # mid-size parity case: several FFT/solver tiles plus ragged tails, oracle finishes in seconds
     "mid": dict(nx=96, ny=65, nz=48, lx=4 * math.pi, lz=2 * math.pi, re=180.0, dt=5e-4, mesh=("cos", 0.8),
                 mean=("reichardt", 180.0), spec="vk", M=8, amp=("rms", 1.0), cut=(11, 7), seed=7),
