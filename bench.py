@@ -46,6 +46,21 @@ SURVEY_GROUPS = {
 }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the ncu --set full capture
+# of profiles/r1e_summary.md (not measured live): keyed by (class, mx, mz, planes per launch).
+NCU_TRAFFIC = {("xfft_prod", 2304, 1728, 5): 0.637543e9 + 0.277069e9, ("zfft_inv", 2304, 1728, 5): 0.424353e9 + 0.597196e9,
+               ("zfft_fwd", 2304, 1728, 5): 0.318561e9 + 0.178629e9}
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 fp64 FMA/clk x 2 x 1965 MHz
+
+
+def xpass_flops_per_point(nx, nz):
+    """"5 N log2 N" flops of the x pass (a4-a6) per grid point: five packed complex transforms of length 3nx/2 plus the
+    products on each of the 3nz/2 rows of a plane."""
+    import math
+    mx, mz = 3 * nx // 2, 3 * nz // 2
+    return mz * (5 * 5.0 * mx * math.log2(mx) + 15.0 * mx) / (nx * nz)
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -294,9 +309,17 @@ def main():
         pts_per_launch = npts
     abytes = BYTES_PER_POINT[dom] * pts_per_launch
     achieved = abytes / (dms / dcnt * 1e-3) / 1e9
+    planes_per_launch = round(pts_per_launch / (c["nx"] * c["nz"]))
     roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
+                "traffic": NCU_TRAFFIC.get((dom, 3 * c["nx"] // 2, 3 * c["nz"] // 2, planes_per_launch)),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
                 "avg_launch_ms": dms / dcnt, "share_of_step": dms / ms_total}
+    if dom == "xfft_prod":
+        # the x pass is bound by shared memory and the fp64 pipe, not by HBM (profiles/r1e_summary.md): second roof
+        fl = xpass_flops_per_point(c["nx"], c["nz"]) * pts_per_launch
+        tf = fl / (dms / dcnt * 1e-3) / 1e12
+        roofline["fp64"] = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
+                            "flops_per_launch": fl, "peak_source": "derived: 148 SM x 64 FMA/clk x 2 x 1.965 GHz"}
     groups = {}
     for gname, (classes, bpp) in SURVEY_GROUPS.items():
         gms = sum(prof[k][0] for k in classes if k in prof)
