@@ -118,6 +118,28 @@ template <int R, bool INV> CHAN_HD void bfly(c2 (&a)[R]) {
     }
 }
 
+// Twiddles of one butterfly, w^k for k = 1..R-1 with w = exp(-2 pi i p/ncur).  CHAN_TW_POWERS: only w is loaded
+// (one 16-byte load) and the powers are formed by at most four successive products each (w2 = w w, w3 = w2 w,
+// w4 = w2 w2, ...; error <= ~5 ulp); otherwise all R-1 come from the table.  With the shared-memory carve-out the
+// transforms need, L1 keeps almost nothing and every table load is an L2 round trip: ncu showed them as the top
+// long-scoreboard stall and ~40% of the memory instructions of the z passes.
+#ifndef CHAN_TW_POWERS
+#define CHAN_TW_POWERS 1
+#endif
+template <int R>
+CHAN_HD void load_twiddles(const FftStage& S, int m, int p, c2 (&tw)[R - 1 > 0 ? R - 1 : 1]) {
+    if constexpr (R >= 2) {
+#if CHAN_TW_POWERS
+        tw[0] = ldtw(S.tw + p);
+#pragma unroll
+        for (int k = 2; k < R; ++k) tw[k - 1] = cmul(tw[k / 2 - 1], tw[k - k / 2 - 1]);     // w^k = w^(k/2) w^(k - k/2)
+#else
+#pragma unroll
+        for (int k = 1; k < R; ++k) tw[k - 1] = ldtw(S.tw + (size_t)(k - 1) * m + p);
+#endif
+    }
+}
+
 // One butterfly of an in-place pass: elements base + k m, k < R, of sequence q.
 //   DIF (inverse direction here): butterfly, then output k times conj(w^k);
 //   DIT (forward direction here): input k times w^k, then butterfly.     w[k-1] = table twiddle (e^{-i}).
@@ -163,10 +185,7 @@ CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int
         const int b = w >> lgT, t = w & (T - 1);
         const int blk = b / m, p = b - blk * m;
         c2 tw[R - 1 > 0 ? R - 1 : 1];
-        if (m > 1) {
-#pragma unroll
-            for (int k = 1; k < R; ++k) tw[k - 1] = ldtw(S.tw + (size_t)(k - 1) * m + p);
-        }
+        if (m > 1) load_twiddles<R>(S, m, p, tw);
         pass_item<R, INV, DIT>(src, dst, t, blk * ncur + p, m, tw, m > 1);
     }
 }
@@ -380,11 +399,8 @@ CHAN_HD void xpass(const XIO& io, const FftStage& S, int n, int nseq, int tid, i
     const int m = M > 0 ? M : S.m, ncur = R * m, nb = n / R;
     for (int b = tid; b < nb; b += nt) {
         const int blk = b / m, p = b - blk * m;
-        c2 tw[R - 1];
-        if (m > 1) {
-#pragma unroll
-            for (int k = 1; k < R; ++k) tw[k - 1] = ldtw(S.tw + (size_t)(k - 1) * m + p);
-        }
+        c2 tw[R - 1 > 0 ? R - 1 : 1];
+        if (m > 1) load_twiddles<R>(S, m, p, tw);
         for (int q = 0; q < nseq; ++q) pass_item<R, INV, DIT>(io, io, q, blk * ncur + p, m, tw, m > 1);
     }
 }
