@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(YNT) k_sa(YParams P, const double2* __restrict
 // SB (descending).  reads zd, H2, phi, h_v^prev, R_om; writes h_v (in place), facA = {1/d, u1},
 // facB = {u2, z_b}, z_phi (over zd), z_om (over R_om).  Helmholtz matrix B2 - lam A2 in orientation 1.
 // =====================================================================================================
-__global__ void __launch_bounds__(YNT) k_sb(YParams P, const double2* __restrict__ H2, const double2* __restrict__ phi,
+__global__ void __launch_bounds__(YNT, 4) k_sb(YParams P, const double2* __restrict__ H2, const double2* __restrict__ phi,
                                             double2* __restrict__ hv, double2* zd_zphi, double2* rom_zom,
                                             double2* __restrict__ facA, double2* __restrict__ facB) {
     __shared__ __align__(16) double sLU[YR * 8], sA2[YR * 8], sB2[YR * 8];
