@@ -391,8 +391,11 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
 CHAN_HD int swz(int e) { return e ^ ((e >> 3) & 7); }
 struct XIO {
     c2* sm; int stride;
-    CHAN_HD c2 load(int e, int q) const { return sm[q * stride + swz(e)]; }
-    CHAN_HD void store(int e, int q, c2 v) const { sm[q * stride + swz(e)] = v; }
+    // zero band of the 3/2 padding, entries blo..bhi: never written by the pack (zin: read as zero by the first
+    // inverse stage) and never needed by the unpack (zout: not written by the last forward stage)
+    int blo = 0, bhi = -1; bool zin = false, zout = false;
+    CHAN_HD c2 load(int e, int q) const { return (zin && e >= blo && e <= bhi) ? mk(0, 0) : sm[q * stride + swz(e)]; }
+    CHAN_HD void store(int e, int q, c2 v) const { if (!(zout && e >= blo && e <= bhi)) sm[q * stride + swz(e)] = v; }
 };
 template <int R, bool INV, bool DIT, int M = 0>
 CHAN_HD void xpass(const XIO& io, const FftStage& S, int n, int nseq, int tid, int nt) {
@@ -463,7 +466,7 @@ CHAN_HD void xfused(const XIO& io, int n, int tid, int nt) {
     }
 }
 
-CHAN_HD void xpack(const XIO& io, int mx, int nxh, const double2* zrow, size_t fstride, int tid, int nt) {
+CHAN_HD void xpack(const XIO& io, int mx, int nxh, const double2* zrow, size_t fstride, int tid, int nt, bool fill_zero) {
     // C[k] = A[k] + i B[k], C[mx-k] = conj(A[k]) + i conj(B[k]); Im of the k = 0 entries dropped (R14)
     for (int w = tid; w < 3 * nxh; w += nt) {
         const int pr = w / nxh, k = w - pr * nxh;
@@ -471,7 +474,7 @@ CHAN_HD void xpack(const XIO& io, int mx, int nxh, const double2* zrow, size_t f
         if (k == 0) io.store(0, pr, mk(A.x, B.x));
         else { io.store(k, pr, mk(A.x - B.y, A.y + B.x)); io.store(mx - k, pr, mk(A.x + B.y, -A.y + B.x)); }
     }
-    const int nzero = mx - 2 * nxh + 1;     // entries nxh .. mx-nxh
+    const int nzero = fill_zero ? mx - 2 * nxh + 1 : 0;     // entries nxh .. mx-nxh (else the first stage reads them as zero)
     for (int w = tid; w < 3 * nzero; w += nt) {
         const int pr = w / nzero, k = w - pr * nzero;
         io.store(nxh + k, pr, mk(0, 0));
@@ -498,13 +501,16 @@ CHAN_HD void xrow_phase(int ph, int tid, int nt, const PlaneParams& P, c2* sm, c
     constexpr int NC = (NPROD + 1) / 2;
     const int mx = P.mx, nxh = P.nxh, ns = P.fx.ns;
     XIO io; io.sm = sm; io.stride = mx;
+    io.blo = nxh; io.bhi = mx - nxh;
     if (ph == 0) {
-        xpack(io, mx, nxh, zrow, fstride, tid, nt);
+        xpack(io, mx, nxh, zrow, fstride, tid, nt, ns == 1);
     } else if (ph < ns) {
+        io.zin = (ph == 1);
         xpass_any<true, false>(io, P.fx.st[ph - 1], mx, 3, tid, nt);
     } else if (ph == ns) {
         xfused<F, NPROD>(io, mx, tid, nt);
     } else if (ph < 2 * ns) {
+        io.zout = (ph == 2 * ns - 1);
         xpass_any<false, true>(io, P.fx.st[2 * ns - 1 - ph], mx, NC, tid, nt);
     } else {
         xunpack<NPROD>(io, mx, xrow, ostride, pout, tid, nt);
@@ -541,16 +547,17 @@ __global__ void __launch_bounds__(256, 2) k_xfft_prod_s(CHAN_XARGS) {
     constexpr int M2 = F, M1 = R2 * F, M0 = R1 * R2 * F, mx = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
     XIO io; io.sm = reinterpret_cast<c2*>(smem_raw); io.stride = mx;
-    xpack(io, mx, P.nxh, zpad + ((size_t)jc * P.mz + r) * P.nxh, (size_t)npl * P.mz * P.nxh, tid, nt);
+    io.blo = mx / 3; io.bhi = mx - mx / 3;
+    xpack(io, mx, P.nxh, zpad + ((size_t)jc * P.mz + r) * P.nxh, (size_t)npl * P.mz * P.nxh, tid, nt, R0 == 1);
     __syncthreads();
-    if constexpr (R0 > 1) { xpass<R0, true, false, M0>(io, P.fx.st[0], mx, 3, tid, nt); __syncthreads(); }
+    if constexpr (R0 > 1) { io.zin = true; xpass<R0, true, false, M0>(io, P.fx.st[0], mx, 3, tid, nt); io.zin = false; __syncthreads(); }
     if constexpr (R1 > 1) { xpass<R1, true, false, M1>(io, P.fx.st[1], mx, 3, tid, nt); __syncthreads(); }
     if constexpr (R2 > 1) { xpass<R2, true, false, M2>(io, P.fx.st[2], mx, 3, tid, nt); __syncthreads(); }
     xfused<F, NPROD>(io, mx, tid, nt);
     __syncthreads();
     if constexpr (R2 > 1) { xpass<R2, false, true, M2>(io, P.fx.st[2], mx, NC, tid, nt); __syncthreads(); }
     if constexpr (R1 > 1) { xpass<R1, false, true, M1>(io, P.fx.st[1], mx, NC, tid, nt); __syncthreads(); }
-    if constexpr (R0 > 1) { xpass<R0, false, true, M0>(io, P.fx.st[0], mx, NC, tid, nt); __syncthreads(); }
+    if constexpr (R0 > 1) { io.zout = true; xpass<R0, false, true, M0>(io, P.fx.st[0], mx, NC, tid, nt); io.zout = false; __syncthreads(); }
     xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
 }
 #endif
