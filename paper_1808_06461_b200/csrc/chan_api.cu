@@ -244,7 +244,9 @@ int xprod(chan_t* h, const PlaneParams& Q, int nprod, int npl, int pout) {
     CK(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
     dim3 g(Q.mz, npl);
     PB(nprod == 3 ? CHAN_KC_XFFT_PROD : CHAN_KC_XFFT_PROD_FILTER);
-    fn<<<g, h->xthreads, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
+    int nt = h->xthreads;
+    if (nprod == 7 && h->xspecial && 2 * (smx + 1024) > 227 * 1024) nt = 512;    // one CTA per SM: fill it
+    fn<<<g, nt, smx, h->stream>>>(Q, h->zpad, npl, h->xh, pout);
     LAUNCHED();
     return CHAN_OK;
 }

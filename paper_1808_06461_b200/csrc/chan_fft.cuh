@@ -539,8 +539,9 @@ __global__ void __launch_bounds__(256, 2) k_xfft_prod_g(CHAN_XARGS) {
 }
 
 // stage radices as template parameters: R0, R1, R2 (1 = absent) then the fused radix F
+// (the filter variant keeps four sequences in shared memory: where only one such CTA fits on an SM it runs 512 threads)
 template <int NPROD, int F, int R0, int R1, int R2>
-__global__ void __launch_bounds__(256, 2) k_xfft_prod_s(CHAN_XARGS) {
+__global__ void __launch_bounds__(NPROD == 7 ? 512 : 256, NPROD == 7 ? 1 : 2) k_xfft_prod_s(CHAN_XARGS) {
     extern __shared__ double2 smem_raw[];
     constexpr int NC = (NPROD + 1) / 2;
     const int r = blockIdx.x, jc = blockIdx.y;
