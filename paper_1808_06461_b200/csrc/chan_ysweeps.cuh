@@ -162,6 +162,7 @@ __global__ void __launch_bounds__(YNT) k_sa(YParams P, const double2* __restrict
     const YS S = ys_setup(P);
     const int ny = P.ny, part = S.part;
     const double c = 1.0 / (P.beta * P.nu * P.dt);
+    const bool hist = (P.zeta != 0.0);
     double wd[7], wt[7], wx[7];
 #pragma unroll
     for (int k = 0; k < 7; ++k) wd[k] = wt[k] = wx[k] = 0.0;
@@ -180,10 +181,10 @@ __global__ void __launch_bounds__(YNT) k_sa(YParams P, const double2* __restrict
             if (jj < nit) {
                 double d = 0.0, x = 0.0, t = 0.0;
                 if (S.act && jj < ny) {
-                    if (jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(H1 + op); pf2(H3 + op); pf2(omy + op); pf2(hg + op); }
+                    if (jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(H1 + op); pf2(H3 + op); pf2(omy + op); if (hist) pf2(hg + op); }
                     const c2 h1 = ldc(H1 + ol), h3 = ldc(H3 + ol);
                     x = *cpart(omy, ol, part);
-                    const double gp = *cpart(hg, ol, part);
+                    const double gp = hist ? *cpart(hg, ol, part) : 0.0;     // zeta_1 = 0: the first substep reads no history
                     // h_g = i kz h1 - i kx h3 ; d = i kx h1 + i kz h3
                     const double g = part ? (S.kz * h1.x - S.kx * h3.x) : (-S.kz * h1.y + S.kx * h3.y);
                     d = part ? (S.kx * h1.x + S.kz * h3.x) : (-S.kx * h1.y - S.kz * h3.y);
@@ -219,6 +220,7 @@ __global__ void __launch_bounds__(YNT, 4) k_sb(YParams P, const double2* __restr
     const YS S = ys_setup(P);
     const int ny = P.ny, part = S.part;
     const double c = 1.0 / (P.beta * P.nu * P.dt), lam = S.k2 + c;
+    const bool hist = (P.zeta != 0.0);
     double wt[7], wx[7];
 #pragma unroll
     for (int k = 0; k < 7; ++k) wt[k] = wx[k] = 0.0;
@@ -230,7 +232,7 @@ __global__ void __launch_bounds__(YNT, 4) k_sb(YParams P, const double2* __restr
     // offset of (row j = ny-1-ii, mode m); runs below zero for the three trailing iterations: signed
     long long ol = (long long)(ny - 1) * P.nm + (S.inplane ? S.m : 0);
     double nzd = 0.0, nh2 = 0.0, nhp = 0.0, nph = 0.0;                    // inputs of the next row, loaded one step ahead
-    if (S.act) { nzd = *cpart(zd_zphi, (size_t)ol, part); nh2 = *cpart(H2, (size_t)ol, part); nhp = *cpart(hv, (size_t)ol, part); nph = *cpart(phi, (size_t)ol, part); }
+    if (S.act) { nzd = *cpart(zd_zphi, (size_t)ol, part); nh2 = *cpart(H2, (size_t)ol, part); nhp = hist ? *cpart(hv, (size_t)ol, part) : 0.0; nph = *cpart(phi, (size_t)ol, part); }
     for (int it0 = 0; it0 < nit; it0 += YR) {
         __syncthreads();
         stage8n(sLU, P.t[0].lu1, ny, it0, ny - 1, -1, YR);        // orientation-0 LU of A1 at physical row j = ny-1-ii
@@ -247,10 +249,10 @@ __global__ void __launch_bounds__(YNT, 4) k_sb(YParams P, const double2* __restr
                 if (S.act && i >= 0) romv = *cpart(rom_zom, oc, part);
                 if (S.act && j >= 0) {
                     const size_t o = (size_t)ol;
-                    if (j - CHAN_PF >= 0) { const size_t op = o - (size_t)CHAN_PF * nm; pf2(zd_zphi + op); pf2(H2 + op); pf2(phi + op); pf2(hv + op); pf2(rom_zom + op); }
+                    if (j - CHAN_PF >= 0) { const size_t op = o - (size_t)CHAN_PF * nm; pf2(zd_zphi + op); pf2(H2 + op); pf2(phi + op); if (hist) pf2(hv + op); pf2(rom_zom + op); }
                     const double zdv = nzd, h2 = nh2, hp = nhp;
                     x = nph;
-                    if (j > 0) { const size_t o1 = o - nm; nzd = *cpart(zd_zphi, o1, part); nh2 = *cpart(H2, o1, part); nhp = *cpart(hv, o1, part); nph = *cpart(phi, o1, part); }
+                    if (j > 0) { const size_t o1 = o - nm; nzd = *cpart(zd_zphi, o1, part); nh2 = *cpart(H2, o1, part); nhp = hist ? *cpart(hv, o1, part) : 0.0; nph = *cpart(phi, o1, part); }
                     const double dd = d1bwd3<R>(bd, sLU + R * 8, zdv);
                     const double h = -S.k2 * h2 - dd;
                     *wpart(hv, o, part) = h;
