@@ -84,7 +84,9 @@ void choose_tiling(chan_t* h) {
     if (const char* e = std::getenv("CHAN_ZTHREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 256) h->zthreads = v; }
     if (const char* e = std::getenv("CHAN_XTHREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 256) h->xthreads = v; }
     const size_t per_plane = (size_t)13 * P.mz * P.nxh * 16;
-    long long pc = (long long)(1536ull * 1024 * 1024 / per_plane);
+    unsigned long long budget = 3072ull << 20;    // zpad + xh: about 11 planes of config 5 per chunk (longer grids, smaller tails)
+    if (const char* e = std::getenv("CHAN_CHUNK_MB")) { const long v = std::atol(e); if (v > 0) budget = (unsigned long long)v << 20; }
+    long long pc = (long long)(budget / per_plane);
     if (pc < 1) pc = 1;
     if (pc > P.ny) pc = P.ny;
     h->pc = (int)pc;
