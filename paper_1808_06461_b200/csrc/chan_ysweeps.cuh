@@ -475,7 +475,7 @@ __global__ void __launch_bounds__(YNT) k_sd0(YParams P, const double2* __restric
 // zw = forward D1(w), both in orientation 0.  u = i (kx dv - kz om_y)/k2, w = i (kz dv + kx om_y)/k2.
 // The z-Nyquist slot is written as zeros (the buffers double as y-phase scratch).
 // =====================================================================================================
-__global__ void __launch_bounds__(YNT) k_se(YParams P, double2* zv_zu, const double2* __restrict__ omy,
+__global__ void __launch_bounds__(YNT, 6) k_se(YParams P, double2* zv_zu, const double2* __restrict__ omy,
                                             const double* __restrict__ U, const double* __restrict__ W,
                                             double2* __restrict__ u, double2* __restrict__ w_, double2* __restrict__ zw) {
     __shared__ __align__(16) double sLUb[YR * 8], sB1[YR * 8], sLU[YR * 8];
