@@ -354,3 +354,28 @@ def test_host_buffer_entry_points(B):
     ch.filter_store_host(8, 8, out)
     assert rel(out, o.filter_store(8, 8)) < 1e-10
     ch.close()
+
+
+def test_unlisted_transform_lengths_use_the_generic_kernels(B):
+    """mx = 72, mz = 27: stage lists ([3,3|8], [3,3,3]) that have no compile-time specialisation, so the run-time
+    radix-switch kernels (k_*_g) carry the planes; one full step, filter and statistics against the oracle."""
+    c = inputs.config("cfg1", nx=48, nz=18, cut=(7, 5))
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind("cuda:0")
+    o = ChannelOracle(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    v, phi, omy = seeded_state(c, 20.0)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    t = make_twin(c)
+    t.set_state(v, phi, omy, c["U"], c["W"])
+    ch.step()
+    o.step()
+    t.step()
+    check_state(ch, o, t, 3, "generic")
+    got = ch.filter_store(*c["cut"]).cpu().numpy()
+    ref = o.filter_store(*c["cut"])
+    for n in range(10):
+        assert rel(got[n], ref[n]) < 1e-10, n
+    ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
+    prof, _ = ch.stats(B.STATS_READ)
+    assert np.abs(prof - o.stats_profiles()).max() < 1e-10 * np.abs(prof).max()
+    ch.close()
