@@ -47,9 +47,9 @@ SURVEY_GROUPS = {
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the ncu --set full capture
-# of profiles/r1e_summary.md (not measured live): keyed by (class, mx, mz, planes per launch).
-NCU_TRAFFIC = {("xfft_prod", 2304, 1728, 5): 0.637543e9 + 0.277069e9, ("zfft_inv", 2304, 1728, 5): 0.424353e9 + 0.597196e9,
-               ("zfft_fwd", 2304, 1728, 5): 0.318561e9 + 0.178629e9}
+# of profiles/r1f_summary.md (not measured live): keyed by (class, mx, mz, planes per launch).
+NCU_TRAFFIC = {("xfft_prod", 2304, 1728, 11): 1.401605e9 + 0.661527e9, ("zfft_inv", 2304, 1728, 11): 0.933496e9 + 1.371144e9,
+               ("zfft_fwd", 2304, 1728, 11): 0.700743e9 + 0.439941e9}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 fp64 FMA/clk x 2 x 1965 MHz
 
 
