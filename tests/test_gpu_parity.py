@@ -379,3 +379,31 @@ def test_unlisted_transform_lengths_use_the_generic_kernels(B):
     prof, _ = ch.stats(B.STATS_READ)
     assert np.abs(prof - o.stats_profiles()).max() < 1e-10 * np.abs(prof).max()
     ch.close()
+
+
+def test_edge_sizes_smallest_grid_and_extreme_cutoffs(B):
+    """Degenerate cases: the smallest grid the ABI accepts (ny = 8: every row of the compact operators is a wall or
+    near-wall row; nx = 16, nz = 4: one tile, one-stage z transform), and the filter at its two extreme cutoffs
+    (only the mean column / every retained mode)."""
+    c = inputs.config("cfg2", ny=8, mesh=("cos", 0.5), dt=1e-3, re=100.0, mean=("poiseuille", 1.0), spec="gauss", M=3,
+                      amp=("maxu", 1e-2), cut=(0, 0), seed=9)
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind("cuda:0")
+    o = ChannelOracle(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    v, phi, omy = seeded_state(c)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    for n in range(3):
+        ch.substep()
+        o.substep()
+    e = state_errors(ch, o)
+    assert max(e["v"], e["phi"], e["omy"], e["U"]) < 3 * TOL_SUBSTEP, e
+    for cut in ((0, 0), (c["nx"] // 2 - 1, c["nz"] // 2 - 1)):
+        got = ch.filter_store(*cut).cpu().numpy()
+        ref = o.filter_store(*cut)
+        assert got.shape == ref.shape == (10, c["ny"], 2 * cut[1] + 1, cut[0] + 1)
+        for n in range(10):
+            assert rel(got[n], ref[n]) < 1e-10, (cut, n)
+    with pytest.raises(B.ChanError) as ex:
+        ch.filter_store(c["nx"] // 2, 0)          # one past the retained range
+    assert ex.value.status == B.EINVAL
+    ch.close()
