@@ -39,7 +39,10 @@ extern "C" {
 typedef struct chan chan_t; /* opaque */
 
 /* nx, nz: Fourier collocation points before the 3/2 padding (even; 3nx/2 and 3nz/2 must factor into
- * 2,3 only); ny: mesh points including both walls (>= 8).  PAPER.md L80. */
+ * 2,3 only; nx a multiple of 16 so that 3nx/2 is a multiple of 8; 3nx/2 <= 3520 and 3nz/2 <= 14080:
+ * one padded x row set / one z column must fit in 220 KB of shared memory); ny: mesh points including
+ * both walls, 8 <= ny <= 1877 (the mean-mode solve keeps 15 ny doubles in shared memory).  Anything else:
+ * CHAN_EINVAL.  PAPER.md L80. */
 typedef struct { int nx, ny, nz; } chan_grid_t;
 
 /* lx, lz: periods; y: HOST array of ny strictly increasing mesh points, y[0] = -1, y[ny-1] = +1.

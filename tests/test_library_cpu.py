@@ -39,6 +39,8 @@ def test_argument_validation_without_gpu(lib):
 
     assert create(33, 33, 32) == binding.EINVAL          # odd nx
     assert create(28, 33, 32) == binding.EINVAL          # 3*28/2 = 42 has a factor 7
+    assert create(24, 33, 32) == binding.EINVAL          # 3*24/2 = 36 is not a multiple of 8 (include/chan.h)
+    assert create(32, 7, 32) == binding.EINVAL           # fewer than 8 mesh points
     assert create(32, 33, 32, re=-1.0) == binding.EINVAL
     yb = y.copy(); yb[5] = yb[4]
     boxb = binding.Box(2 * np.pi, np.pi, yb.ctypes.data_as(C.POINTER(C.c_double)))
