@@ -108,6 +108,13 @@ int chan_set_pgrad(chan_t* h, double minus_dpdx); /* forcing == 1 only */
 
 const char* chan_strerror(int status);
 
+/* ---- tuning overrides ---------------------------------------------------------------------------
+ * chan_create() reads these environment variables once (unset = the plan's own choice); they change
+ * launch geometry and stage lists, never results beyond rounding:
+ *   CHAN_XFUSE=4|8      radix of the x stage fused with the products      CHAN_MAXRADIX=2..12  largest stage radix
+ *   CHAN_TZ=1..16       k_x columns per z tile (power of two)              CHAN_ZTHREADS, CHAN_XTHREADS  threads per CTA
+ *   CHAN_CHUNK_MB       size of the z-padded plane-chunk buffers (default 3072) */
+
 /* ---- debug / parity / profiling hooks (run one stage on library buffers) ------------------------
  * Field ids for chan_debug_get_field / chan_debug_set_field (LINE layout, device pointers): */
 enum { CHAN_F_V = 0, CHAN_F_PHI, CHAN_F_OMY, CHAN_F_U, CHAN_F_W, CHAN_F_OMX, CHAN_F_OMZ,
