@@ -111,7 +111,7 @@ const char* chan_strerror(int status);
 /* ---- tuning overrides ---------------------------------------------------------------------------
  * chan_create() reads these environment variables once (unset = the plan's own choice); they change
  * launch geometry and stage lists, never results beyond rounding:
- *   CHAN_XFUSE=4|8      radix of the x stage fused with the products      CHAN_MAXRADIX=2..12  largest stage radix
+ *   CHAN_XFUSE=4|8      radix of the x stage fused with the products      CHAN_MAXRADIX=2..12  largest stage radix (CHAN_MAXRADIX_X=2..16: x pass only)
  *   CHAN_TZ=1..16       k_x columns per z tile (power of two)              CHAN_ZTHREADS, CHAN_XTHREADS  threads per CTA
  *   CHAN_CHUNK_MB       size of the z-padded plane-chunk buffers (default 3072) */
 

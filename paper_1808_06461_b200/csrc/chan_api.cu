@@ -189,7 +189,7 @@ int run_derive(chan_t* h) {
     X(6, 8, 8, 4) X(6, 6, 8, 8) X(6, 8, 8, 8)
 #define CHAN_XPLANS(X) X(4, 6, 1, 1) X(4, 12, 1, 1) X(4, 6, 4, 1) X(4, 6, 6, 1) X(4, 6, 8, 1) X(4, 12, 8, 1) X(4, 6, 6, 4) X(4, 6, 6, 6) \
     X(4, 6, 8, 4) X(4, 6, 6, 8) X(4, 6, 8, 8) X(4, 12, 6, 6) X(4, 12, 6, 8) X(4, 12, 8, 8) X(8, 6, 1, 1) X(8, 12, 1, 1) X(8, 12, 6, 1) \
-    X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
+    X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 12, 16, 1) X(8, 16, 1, 1) X(8, 12, 8, 1) X(8, 6, 6, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
 
 typedef void (*zinv_fn)(PlaneParams, FieldPtrs, int, int, double2*, int);
 typedef void (*zfwd_fn)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int);

@@ -3,7 +3,7 @@
 // ("pseudo-spectral ... fully dealiased by zero padding"), L84 (batched plane FFTs), L124 (filter).
 //
 // Transform engine.  A length-n transform (n = 2^a 3^b) is a list of register-resident stages of radix
-// 2,3,4,6,8 or 12 (chan_plan.cpp chooses them), run IN PLACE in shared memory:
+// 2,3,4,6,8,12 (and 16 in the x pass; chan_plan.cpp chooses them), run IN PLACE in shared memory:
 //   spectral -> physical: decimation in frequency, e^{+i}, natural order in, digit-reversed order out;
 //   physical -> spectral: decimation in time, e^{-i}, the same stage list backwards.
 // Physical space is only ever used pointwise, so the digit-reversed order is never undone.
@@ -77,8 +77,28 @@ template <bool INV> CHAN_HD void dft4(c2& a0, c2& a1, c2& a2, c2& a3) {
     a0 = s0 + s1; a2 = s0 - s1; a1 = d0 + jd; a3 = d0 - jd;
 }
 
+// a * exp(-i t) (forward) or a * exp(+i t) (inverse), c = cos t, s = sin t
+template <bool INV> CHAN_HD c2 mulcs(c2 a, double c, double s) {
+    return INV ? mk(a.x * c - a.y * s, a.x * s + a.y * c) : mk(a.x * c + a.y * s, a.y * c - a.x * s);
+}
+// radix 16 = 4 x 4 (Cooley-Tukey, twiddles w16^(n2 k1))
+template <bool INV> CHAN_HD void dft16(c2 (&a)[16]) {
+    const double c1 = 0.92387953251128675613, s1 = 0.38268343236508977173, h = 0.70710678118654752440;   // pi/8, pi/4
+    c2 y[4][4];
+#pragma unroll
+    for (int n2 = 0; n2 < 4; ++n2) { c2 p = a[n2], q = a[4 + n2], r = a[8 + n2], s = a[12 + n2]; dft4<INV>(p, q, r, s); y[0][n2] = p; y[1][n2] = q; y[2][n2] = r; y[3][n2] = s; }
+    // w16^(n2 k1), angles n2 k1 pi/8
+    y[1][1] = mulcs<INV>(y[1][1], c1, s1); y[1][2] = mulcs<INV>(y[1][2], h, h); y[1][3] = mulcs<INV>(y[1][3], s1, c1);
+    y[2][1] = mulcs<INV>(y[2][1], h, h); y[2][2] = rot90<INV>(y[2][2]); y[2][3] = mulcs<INV>(y[2][3], -h, h);
+    y[3][1] = mulcs<INV>(y[3][1], s1, c1); y[3][2] = mulcs<INV>(y[3][2], -h, h); y[3][3] = mulcs<INV>(y[3][3], -c1, -s1);
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) { c2 p = y[k1][0], q = y[k1][1], r = y[k1][2], s = y[k1][3]; dft4<INV>(p, q, r, s); a[k1] = p; a[k1 + 4] = q; a[k1 + 8] = r; a[k1 + 12] = s; }
+}
+
 template <int R, bool INV> CHAN_HD void bfly(c2 (&a)[R]) {
-    if constexpr (R == 2) {
+    if constexpr (R == 16) {
+        dft16<INV>(a);
+    } else if constexpr (R == 2) {
         dft2<INV>(a[0], a[1]);
     } else if constexpr (R == 3) {
         dft3<INV>(a[0], a[1], a[2]);
@@ -128,7 +148,9 @@ template <int R, bool INV> CHAN_HD void bfly(c2 (&a)[R]) {
 #endif
 template <int R>
 CHAN_HD void load_twiddles(const FftStage& S, int m, int p, c2 (&tw)[R - 1 > 0 ? R - 1 : 1]) {
-    if constexpr (R >= 2) {
+    if constexpr (R > 12) {
+        tw[0] = ldtw(S.tw + p);         // radix 16: pass_item forms w^k on the fly (a register file of 15 powers would spill)
+    } else if constexpr (R >= 2) {
 #if CHAN_TW_POWERS
         tw[0] = ldtw(S.tw + p);
 #pragma unroll
@@ -148,14 +170,29 @@ CHAN_HD void pass_item(const Src& src, const Dst& dst, int q, int base, int m, c
     c2 a[R];
 #pragma unroll
     for (int k = 0; k < R; ++k) a[k] = src.load(base + k * m, q);
-    if (DIT && twiddled) {
+    if constexpr (R > 12) {
+        const c2 w1 = INV ? mk(w[0].x, -w[0].y) : w[0];
+        if (DIT && twiddled) {
+            c2 wk = w1;
 #pragma unroll
-        for (int k = 1; k < R; ++k) a[k] = cmul(a[k], INV ? mk(w[k - 1].x, -w[k - 1].y) : w[k - 1]);
-    }
-    bfly<R, INV>(a);
-    if (!DIT && twiddled) {
+            for (int k = 1; k < R; ++k) { a[k] = cmul(a[k], wk); if (k + 1 < R) wk = cmul(wk, w1); }
+        }
+        bfly<R, INV>(a);
+        if (!DIT && twiddled) {
+            c2 wk = w1;
 #pragma unroll
-        for (int k = 1; k < R; ++k) a[k] = cmul(a[k], INV ? mk(w[k - 1].x, -w[k - 1].y) : w[k - 1]);
+            for (int k = 1; k < R; ++k) { a[k] = cmul(a[k], wk); if (k + 1 < R) wk = cmul(wk, w1); }
+        }
+    } else {
+        if (DIT && twiddled) {
+#pragma unroll
+            for (int k = 1; k < R; ++k) a[k] = cmul(a[k], INV ? mk(w[k - 1].x, -w[k - 1].y) : w[k - 1]);
+        }
+        bfly<R, INV>(a);
+        if (!DIT && twiddled) {
+#pragma unroll
+            for (int k = 1; k < R; ++k) a[k] = cmul(a[k], INV ? mk(w[k - 1].x, -w[k - 1].y) : w[k - 1]);
+        }
     }
 #pragma unroll
     for (int k = 0; k < R; ++k) dst.store(base + k * m, q, a[k]);
@@ -197,6 +234,7 @@ CHAN_HD void zpass_any(const Src& src, const Dst& dst, const FftStage& S, int n,
         case 4: zpass<4, INV, DIT>(src, dst, S, n, T, tid, nt); break;
         case 6: zpass<6, INV, DIT>(src, dst, S, n, T, tid, nt); break;
         case 8: zpass<8, INV, DIT>(src, dst, S, n, T, tid, nt); break;
+        case 16: zpass<16, INV, DIT>(src, dst, S, n, T, tid, nt); break;
         default: zpass<12, INV, DIT>(src, dst, S, n, T, tid, nt); break;
     }
 }
@@ -415,6 +453,7 @@ CHAN_HD void xpass_any(const XIO& io, const FftStage& S, int n, int nseq, int ti
         case 4: xpass<4, INV, DIT>(io, S, n, nseq, tid, nt); break;
         case 6: xpass<6, INV, DIT>(io, S, n, nseq, tid, nt); break;
         case 8: xpass<8, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        case 16: xpass<16, INV, DIT>(io, S, n, nseq, tid, nt); break;
         default: xpass<12, INV, DIT>(io, S, n, nseq, tid, nt); break;
     }
 }

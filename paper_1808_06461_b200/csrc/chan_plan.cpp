@@ -166,15 +166,15 @@ void pad8(int ny, const std::vector<double>& T, std::vector<double>& O) {
 
 // Stage list for length n = 2^a 3^b (chan_fft.cuh).  `fused_last` > 0 fixes the last radix (the x
 // transform fuses that stage with the pointwise products); the rest is the shortest list of radices from
-// {12,8,6,4,3,2} (fewest radix-12 stages among the shortest), radices with a factor 3 first so that the
+// {16,12,8,6,4,3,2} (fewest radix-12/16 stages among the shortest), radices with a factor 3 first so that the
 // zero band of the 3/2 padding lines up with whole inputs of the first butterfly.
 void best_radices(int rest, int maxr, std::vector<int>& cur, std::vector<int>& best) {
-    static const int cand[6] = {12, 8, 6, 4, 3, 2};
+    static const int cand[7] = {16, 12, 8, 6, 4, 3, 2};
     if (rest == 1) {
         auto key = [](const std::vector<int>& v) {
-            int c12 = 0, c2 = 0;
-            for (int r : v) { c12 += (r == 12); c2 += (r <= 3); }
-            return (long)v.size() * 10000 + c12 * 100 + c2;
+            int big = 0, c2 = 0, mx = 0;
+            for (int r : v) { big += (r == 12) + 2 * (r > 12); c2 += (r <= 3); mx = r > mx ? r : mx; }
+            return (long)v.size() * 100000 + big * 1000 + mx * 10 + c2;
         };
         if (best.empty() || key(cur) < key(best)) best = cur;
         return;
@@ -251,19 +251,24 @@ int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const doub
     const char* ef = std::getenv("CHAN_XFUSE");
     const char* er = std::getenv("CHAN_MAXRADIX");
     const int maxr = (er && std::atoi(er) >= 2) ? std::atoi(er) : 12;
+    // the x pass may use radix 16 (two shared-memory stages in front of the fused one at 1536 points; radix 18, which
+    // would do the same at 2304 points, was measured slower: it spills ~400 bytes under the 128-register cap);
+    // the z passes stay at 12
+    const char* erx = std::getenv("CHAN_MAXRADIX_X");
+    const int maxrx = er ? maxr : ((erx && std::atoi(erx) >= 2) ? std::atoi(erx) : 16);
     int fuse = 4;
     if (ef) fuse = (std::atoi(ef) == 8) ? 8 : 4;
     else {   // the fused radix (4 or 8) that gives the shorter stage list, then the one without radix-12 stages
              // (they spill under the 128-register cap), then 4 (lighter fused stage)
         FftPlan f4, f8;
         auto key = [](const FftPlan& f) {
-            int c12 = 0;
-            for (int r : f.radix) c12 += (r == 12);
-            return (int)f.radix.size() * 100 + c12;
+            int big = 0;
+            for (int r : f.radix) big += (r == 12) + 3 * (r > 12);
+            return (int)f.radix.size() * 100 + big;
         };
-        if (make_fft_plan(P.mx, 4, maxr, f4) && make_fft_plan(P.mx, 8, maxr, f8) && key(f8) < key(f4)) fuse = 8;
+        if (make_fft_plan(P.mx, 4, maxrx, f4) && make_fft_plan(P.mx, 8, maxrx, f8) && key(f8) < key(f4)) fuse = 8;
     }
-    if (!make_fft_plan(P.mx, fuse, maxr, P.fx) || !make_fft_plan(P.mz, 0, maxr, P.fz)) return CHAN_EINVAL;
+    if (!make_fft_plan(P.mx, fuse, maxrx, P.fx) || !make_fft_plan(P.mz, 0, maxr, P.fz)) return CHAN_EINVAL;
 
     // RK3 constants of [34] (reading R3)
     const double al[3] = {29.0 / 96.0, -3.0 / 40.0, 1.0 / 6.0}, be[3] = {37.0 / 160.0, 5.0 / 24.0, 1.0 / 6.0};
