@@ -117,9 +117,10 @@ def test_d1_on_smooth_function():
     assert np.abs(g - 2 * np.cos(2 * y)).max() < 5e-9  # wall rows are 4th order
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "mid"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "mid", "cfg3", "cfg4", "cfg5"])
 def test_d2_dirichlet_spectrum_admissible(name):
-    """PAPER.md section 2.3 (L100-102): wide stencils are only usable on a mesh they were checked on.
+    """PAPER.md section 2.3 (L100-102): wide stencils are only usable on a mesh they were checked on (every mesh
+    bench.py times is checked here: SURVEY.md Appendix A "harness obligation").
     Generalised eigenvalues of (B2, A2) with Dirichlet walls must be real, negative, -> -(n pi/2)^2."""
     import scipy.linalg as sla
     c = inputs.config(name)
