@@ -407,3 +407,28 @@ def test_edge_sizes_smallest_grid_and_extreme_cutoffs(B):
         ch.filter_store(c["nx"] // 2, 0)          # one past the retained range
     assert ex.value.status == B.EINVAL
     ch.close()
+
+
+def test_constant_pressure_gradient_forcing_and_narrow_stencils(B):
+    """chan_opts_t: forcing = 1 (prescribed -dP/dx instead of the constant mass flux of PAPER.md L61) and the narrower
+    compact schemes of reading R4 (half widths 2/2: the same kernels with zeros in the band tables)."""
+    c = inputs.config("cfg1")
+    v, phi, omy = seeded_state(c, 20.0)
+    for forcing, hl, hr in ((1, 3, 3), (0, 2, 2)):
+        ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"], forcing=forcing, half_lhs=hl,
+                       half_rhs=hr).bind("cuda:0")
+        o = ChannelOracle(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"], forcing=forcing, half_lhs=hl,
+                          half_rhs=hr)
+        ch.set_state(v, phi, omy, c["U"], c["W"])
+        o.set_state(v, phi, omy, c["U"], c["W"])
+        if forcing:
+            ch.set_pgrad(1.25)
+            o.pgrad = 1.25
+        for _ in range(3):
+            ch.substep()
+            o.substep()
+        e = state_errors(ch, o)
+        assert max(e["v"], e["omy"], e["U"]) < 3 * TOL_SUBSTEP, (forcing, hl, e)
+        assert e["phi"] < 1e-9, (forcing, hl, e)
+        assert ch.scalars()[0] == pytest.approx(o.pgrad, rel=1e-9)
+        ch.close()
