@@ -28,7 +28,11 @@ def _worker(rank, world, port, out):
 
 
 def test_max_over_ranks_and_job_value_gloo(tmp_path):
-    world, port = 2, 29541
+    import socket
+    with socket.socket() as sk:                 # a free port for the rendezvous on 127.0.0.1
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    world = 2
     out = str(tmp_path / "r")
     mp.spawn(_worker, args=(world, port, out), nprocs=world, join=True)
     res = [json.load(open(out + f".{r}")) for r in range(world)]
