@@ -165,6 +165,50 @@ def oracle_sample(cfg_name, steps, warmup):
     return 3 * pts * steps / dt / 1e6, dt / steps * 1e3, sample
 
 
+def cufft_reference_line(c, dev, npl=8):
+    """Context only (north_star: "cuFFT may be timed only as a reference line, not used in the product"): the same plane
+    transforms of one substep -- 6 fields spectral -> physical with 3/2 padding, 3 fields back with truncation -- through
+    torch.fft (cuFFT, complex128) on a chunk of `npl` planes, scaled to the ny planes of the workload.  No products."""
+    import torch
+    nx, nz, ny = c["nx"], c["nz"], c["ny"]
+    nxh, mx, mz = nx // 2, 3 * nx // 2, 3 * nz // 2
+    g = torch.Generator(device=dev).manual_seed(1)
+    x = torch.view_as_complex(torch.randn((npl, nz, nxh, 2), generator=g, dtype=torch.float64, device=dev))
+    pad = torch.zeros((npl, mz, mx // 2 + 1), dtype=torch.complex128, device=dev)
+
+    def inverse(f):
+        pad.zero_()
+        pad[:, : nz // 2, :nxh] = f[:, : nz // 2]
+        pad[:, mz - (nz // 2 - 1):, :nxh] = f[:, nz // 2 + 1:]
+        return torch.fft.irfft(torch.fft.ifft(pad, dim=1), n=mx, dim=2)
+
+    def forward(r):
+        s = torch.fft.fft(torch.fft.rfft(r, dim=2)[:, :, :nxh], dim=1)
+        return torch.cat([s[:, : nz // 2], s[:, :1] * 0, s[:, mz - (nz // 2 - 1):]], dim=1)
+
+    for _ in range(3):
+        ph = inverse(x)
+        forward(ph)
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    torch.cuda.synchronize(dev)
+    e[0].record()
+    for _ in range(6):
+        ph = inverse(x)
+    e[1].record()
+    for _ in range(3):
+        forward(ph)
+    e[2].record()
+    for _ in range(6):      # the two inverse transforms alone, no padding copies
+        torch.fft.irfft(torch.fft.ifft(pad[:, :, :nxh], dim=1), n=mx, dim=2)
+    e[3].record()
+    torch.cuda.synchronize(dev)
+    k = ny / npl
+    return {"what": "torch.fft (cuFFT) complex128, same padded plane transforms of one substep, products excluded",
+            "ms_per_substep": (e[0].elapsed_time(e[1]) + e[1].elapsed_time(e[2])) * k,
+            "inverse_6_fields_ms": e[0].elapsed_time(e[1]) * k, "forward_3_fields_ms": e[1].elapsed_time(e[2]) * k,
+            "inverse_transforms_alone_ms": e[2].elapsed_time(e[3]) * k, "planes_timed": npl}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -197,6 +241,7 @@ def main():
     ap.add_argument("--workload", default="auto")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft-line", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -377,6 +422,14 @@ def main():
             dist.destroy_process_group()
         return
 
+    cufft = None
+    if world == 1 and not args.no_cufft_line:
+        try:
+            cufft = cufft_reference_line(c, dev)
+            cufft["ours_ms_per_substep"] = sum(prof[k][0] for k in ("xfft_prod", "zfft_fwd") if k in prof) / (3 * K) \
+                + (prof["zfft_inv"][0] / (4 * K) if "zfft_inv" in prof else 0.0)
+        except RuntimeError as ex:
+            cufft = {"error": str(ex)[:200]}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         val, ms, sample = oracle_sample(wl, 1, 0)
@@ -393,7 +446,7 @@ def main():
                    "workspace_GB": ws_bytes / 1e9, "multi_gpu": "replicas only", "state_finite": finite},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches),
         "substep_only": substep_only, "roofline": roofline, "roofline_groups": groups, "kernel_ms": kernel_ms,
-        "cpu_baseline": cpu,
+        "cpu_baseline": cpu, "cufft_reference_line": cufft,
     }
     print(json.dumps(line))
     if world > 1:
