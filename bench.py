@@ -1,9 +1,9 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the channel-flow hot path on B200 (metric: BASELINE.json).
 
-A "step" is one pass of the whole hot path over one synthetic field: one full RK3 step
-(3 x chan_substep = rows a1-a12 of DESIGN.md), one chan_filter_store (a13) and one chan_stats
-accumulate (a14).  ``value`` counts only the 3 substeps' grid points (Mpoint*RK-substeps/s), so the
+A "step" is one pass of the whole hot path over one synthetic field: one chan_stats accumulate (a14) and
+one chan_step_filter = the filtered database of the entry state (a13) fused into one full RK3 step
+(3 substeps = rows a1-a12 of DESIGN.md).  ``value`` counts only the 3 substeps' grid points (Mpoint*RK-substeps/s), so the
 filter and statistics time is inside the denominator but earns no credit; ``substep_only`` gives the
 rate of the substeps alone.  Inputs are resident in HBM before the timed region; ``e2e`` repeats the
 measurement through the *_host entry points with pinned host buffers (state in, state + filtered
@@ -293,9 +293,10 @@ def main():
     stream = ch.stream
 
     def one_step():
-        ch.step()
-        ch.filter_store(kxc, kzc, fout)
+        # statistics and filtered database of the state the step starts from, then the step: chan_step_filter forms the
+        # filter products from the z-padded planes of the first substep (no inverse z sweep of its own)
         ch.stats(binding.STATS_ACCUMULATE)
+        ch.step_filter(kxc, kzc, fout)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -343,9 +344,8 @@ def main():
     dms, dcnt = sub_classes[dom]
     launches_per_field = dcnt / K          # per step
     # points one launch processes: y-phase kernels and stats see the whole field; plane kernels one chunk
-    uses = {"zfft_inv": 4, "xfft_prod": 3, "zfft_fwd": 3}.get(dom, None)   # field sweeps per step (3 substeps [+ filter])
     if dom in ("zfft_inv",):
-        pts_per_launch = npts * 4 / launches_per_field
+        pts_per_launch = npts * 3 / launches_per_field      # 3 sweeps per step: the fused filter shares the first one
     elif dom in ("xfft_prod", "zfft_fwd"):
         pts_per_launch = npts * 3 / launches_per_field
     elif dom == "stats":
@@ -371,12 +371,6 @@ def main():
         if gms > 0:
             gb = bpp * npts * 3 * K / (gms * 1e-3) / 1e9     # substep part only: the filter has its own classes
             groups[gname] = {"ms_per_substep": gms / (3 * K), "survey_bytes_per_point": bpp, "achieved_GBs": gb, "frac": gb / peak}
-    # the zfft_inv class is also used by the filter (one extra sweep per step): scale its group to 4 sweeps
-    if "K2 z-pad + inverse z-FFT" in groups:
-        g = groups["K2 z-pad + inverse z-FFT"]
-        g["achieved_GBs"] *= 4.0 / 3.0
-        g["frac"] *= 4.0 / 3.0
-        g["ms_per_substep"] *= 3.0 / 4.0
     kernel_ms = {k: {"ms_per_step": v_[0] / K, "launches_per_step": v_[1] / K} for k, v_ in sub_classes.items()}
 
     # ---- end to end through the host-buffer entry points ---------------------------------------------
@@ -427,7 +421,7 @@ def main():
         try:
             cufft = cufft_reference_line(c, dev)
             cufft["ours_ms_per_substep"] = sum(prof[k][0] for k in ("xfft_prod", "zfft_fwd") if k in prof) / (3 * K) \
-                + (prof["zfft_inv"][0] / (4 * K) if "zfft_inv" in prof else 0.0)
+                + (prof["zfft_inv"][0] / (3 * K) if "zfft_inv" in prof else 0.0)
         except RuntimeError as ex:
             cufft = {"error": str(ex)[:200]}
     cpu = None
@@ -441,7 +435,7 @@ def main():
         "ms_per_step": ms_total_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl, "grid": [c["nx"], c["ny"], c["nz"]], "padded": [3 * c["nx"] // 2, c["ny"], 3 * c["nz"] // 2],
-                   "step": "1 RK3 step (3 chan_substep) + chan_filter_store + chan_stats(ACCUMULATE); value counts the 3 substeps",
+                   "step": "chan_stats(ACCUMULATE) + chan_step_filter (= chan_filter_store of the entry state + 1 RK3 step of 3 substeps); value counts the 3 substeps",
                    "filter_cut": [kxc, kzc], "l2": "inputs larger than L2 (one field = %.2f GB)" % (F / 1e9),
                    "workspace_GB": ws_bytes / 1e9, "multi_gpu": "replicas only", "state_finite": finite},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches),

@@ -89,6 +89,10 @@ int chan_step(chan_t* h);
  * restricted to 0<=p<=kx_cut, |q|<=kz_cut into dev_out[10][ny][2 kz_cut+1][kx_cut+1] complex128
  * (z rows ordered q = 0..kz_cut, -kz_cut..-1).  Products are formed on the dealiased grid. */
 int chan_filter_store(chan_t* h, int kx_cut, int kz_cut, void* dev_out, size_t out_bytes);
+/* chan_filter_store of the CURRENT state fused into the full step that follows: identical output and identical new
+ * state (bit for bit) as chan_filter_store() then chan_step(), but the filter products are formed from the z-padded
+ * planes the first substep computes anyway, which saves the filter's own inverse z sweep.  CHAN_ESTATE mid-step. */
+int chan_step_filter(chan_t* h, int kx_cut, int kz_cut, void* dev_out, size_t out_bytes);
 /* Same with a HOST output buffer (synchronises).  The output is staged in one scratch field of the workspace:
  * CHAN_ENOSPACE if it is larger than max(one field, min(ten fields, 64 MiB)) -- use chan_filter_store then. */
 int chan_filter_store_host(chan_t* h, int kx_cut, int kz_cut, void* host_out, size_t out_bytes);

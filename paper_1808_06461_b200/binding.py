@@ -21,7 +21,7 @@ STAGE_DERIVE, STAGE_NONLINEAR, STAGE_YSOLVE = range(3)
 EXPORTS = [
     "chan_create", "chan_destroy", "chan_workspace_bytes", "chan_bind", "chan_set_state", "chan_get_state",
     "chan_set_state_host", "chan_get_state_host", "chan_substep", "chan_step", "chan_filter_store",
-    "chan_filter_store_host", "chan_stats", "chan_get_scalars", "chan_set_pgrad", "chan_strerror",
+    "chan_filter_store_host", "chan_step_filter", "chan_stats", "chan_get_scalars", "chan_set_pgrad", "chan_strerror",
     "chan_debug_get_field", "chan_debug_set_field", "chan_debug_run_stage", "chan_debug_set_substep_index",
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
     "chan_debug_profile", "chan_debug_profile_read",
@@ -72,6 +72,7 @@ def load():
         "chan_step": (i, [vp]),
         "chan_filter_store": (i, [vp, i, i, vp, sz]),
         "chan_filter_store_host": (i, [vp, i, i, vp, sz]),
+        "chan_step_filter": (i, [vp, i, i, vp, sz]),
         "chan_stats": (i, [vp, i, vp, C.POINTER(C.c_longlong)]),
         "chan_get_scalars": (i, [vp, vp]),
         "chan_set_pgrad": (i, [vp, d]),
@@ -169,6 +170,14 @@ class Channel:
         if out is None:
             out = torch.empty(shape, dtype=torch.complex128, device=self.device)
         _chk(self.lib.chan_filter_store(self.h, kx_cut, kz_cut, out.data_ptr(), out.numel() * 16), "chan_filter_store")
+        return out
+
+    def step_filter(self, kx_cut, kz_cut, out=None):
+        """filter_store of the current state fused into the step that follows."""
+        shape = (10, self.ny, 2 * kz_cut + 1, kx_cut + 1)
+        if out is None:
+            out = torch.empty(shape, dtype=torch.complex128, device=self.device)
+        _chk(self.lib.chan_step_filter(self.h, kx_cut, kz_cut, out.data_ptr(), out.numel() * 16), "chan_step_filter")
         return out
 
     def filter_store_host(self, kx_cut, kz_cut, out):

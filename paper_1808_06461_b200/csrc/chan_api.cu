@@ -272,6 +272,27 @@ int run_planes(chan_t* h, int nprod, const FieldPtrsW& out, int kxc, int kzc) {
     return CHAN_OK;
 }
 
+// a3-a8 and the product part of a13 from the SAME z-padded chunks: the filter of the state a substep starts from
+// costs no inverse z sweep of its own
+int run_planes_both(chan_t* h, const FieldPtrsW& outH, const FieldPtrsW& outF, int kxc, int kzc) {
+    const Plan& P = h->P;
+    PlaneParams Q = pparams(h);
+    FieldPtrs in;
+    in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w; in.f[3] = h->ox; in.f[4] = h->omy; in.f[5] = h->oz;
+    const double scale = 1.0 / ((double)P.mx * (double)P.mz);
+    for (int j0 = 0; j0 < P.ny; j0 += h->pc) {
+        const int npl = (P.ny - j0 < h->pc) ? P.ny - j0 : h->pc;
+        int rc = zinv(h, Q, in, 6, j0, npl);
+        if (rc) return rc;
+        // the filter products first: its z pass reads the small xh, then the H pass overwrites xh and (later) u, w, om_x
+        if ((rc = xprod(h, Q, 7, npl, kxc + 1))) return rc;
+        if ((rc = zfwd(h, Q, kxc + 1, 7, j0, npl, outF, scale, 1, kxc, kzc))) return rc;
+        if ((rc = xprod(h, Q, 3, npl, P.nxh))) return rc;
+        if ((rc = zfwd(h, Q, P.nxh, 3, j0, npl, outH, scale, 0, 0, 0))) return rc;
+    }
+    return CHAN_OK;
+}
+
 int run_nonlinear(chan_t* h) {
     FieldPtrsW out;
     out.f[0] = h->H1; out.f[1] = h->H2; out.f[2] = h->H3;
@@ -468,6 +489,29 @@ int chan_filter_store(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_byt
     FieldPtrsW o;
     for (int k = 0; k < 7; ++k) o.f[k] = out + (size_t)(3 + k) * per;
     return run_planes(h, 7, o, kxc, kzc);
+}
+
+int chan_step_filter(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
+    if (!h || !dev_out) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state || h->isub != 0) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
+    const size_t per = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1);
+    if (out_bytes < per * 10 * 16) return CHAN_ENOSPACE;
+    double2* out = (double2*)dev_out;
+    PlaneParams Q = pparams(h);
+    FieldPtrs in; in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w;
+    PB(CHAN_KC_FILTER_COPY); k_filter_copy<<<296, 256, 0, h->stream>>>(Q, in, out, kxc, kzc); LAUNCHED();
+    FieldPtrsW oF, oH;
+    for (int k = 0; k < 7; ++k) oF.f[k] = out + (size_t)(3 + k) * per;
+    oH.f[0] = h->H1; oH.f[1] = h->H2; oH.f[2] = h->H3;
+    int rc;
+    if ((rc = run_planes_both(h, oH, oF, kxc, kzc))) return rc;
+    if ((rc = run_ysolve(h))) return rc;
+    h->isub = 1;
+    if ((rc = run_derive_tail(h))) return rc;
+    for (int i = 1; i < 3; ++i) if ((rc = chan_substep(h))) return rc;
+    return CHAN_OK;
 }
 
 int chan_filter_store_host(chan_t* h, int kxc, int kzc, void* host_out, size_t out_bytes) {

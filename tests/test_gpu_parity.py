@@ -432,3 +432,29 @@ def test_constant_pressure_gradient_forcing_and_narrow_stencils(B):
         assert e["phi"] < 1e-9, (forcing, hl, e)
         assert ch.scalars()[0] == pytest.approx(o.pgrad, rel=1e-9)
         ch.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mid"])
+def test_step_filter_is_filter_store_then_step_bit_for_bit(B, name):
+    """chan_step_filter: same database and same new state as the two separate calls."""
+    c = inputs.config(name)
+    v, phi, omy = seeded_state(c, 20.0 if name == "cfg1" else 1.0)
+    outs = []
+    for fused in (False, True):
+        ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind("cuda:0")
+        ch.set_state(v, phi, omy, c["U"], c["W"])
+        ch.step()
+        if fused:
+            db = ch.step_filter(*c["cut"])
+        else:
+            db = ch.filter_store(*c["cut"])
+            ch.step()
+        outs.append([db.clone()] + [t.clone() for t in ch.get_state()])
+        if fused:
+            ch.substep()
+            with pytest.raises(B.ChanError) as ex:
+                ch.step_filter(*c["cut"])         # mid-step
+            assert ex.value.status == B.ESTATE
+        ch.close()
+    for a, b in zip(*outs):
+        assert torch.equal(a, b)
