@@ -383,9 +383,10 @@ def main():
 
             def e2e_step():
                 ch.set_state_host(hv, hp, ho, hU, hW)
-                ch.step()
-                ch.filter_store_host(kxc, kzc, hf)
                 ch.stats(binding.STATS_ACCUMULATE | binding.STATS_READ)
+                ch.step_filter(kxc, kzc, fout)
+                with torch.cuda.stream(stream):
+                    hf.copy_(fout)                      # the filtered database back to pinned host memory
                 ch.get_state_host(hv, hp, ho, hU, hW)
 
             e2e_step()
@@ -403,7 +404,7 @@ def main():
             e2e = {"value": job_value(npts, 3 * Ke, world, ms_e), "unit": UNIT, "steps": Ke,
                    "ms_per_step": ms_e / Ke, "h2d_bytes_per_step": state_b,
                    "d2h_bytes_per_step": state_b + hf.numel() * 16 + 10 * c["ny"] * 8,
-                   "api": "chan_set_state_host + chan_step + chan_filter_store_host + chan_stats(READ) + chan_get_state_host, "
+                   "api": "chan_set_state_host + chan_stats(READ) + chan_step_filter + database D2H + chan_get_state_host, "
                           + ("pinned" if pinned else "pageable (pinning refused)") + " host buffers"}
             del hf
         except RuntimeError as ex:      # pinned allocation refused by the host
