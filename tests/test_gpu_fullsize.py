@@ -69,7 +69,10 @@ def take_lines(t, ps, ss):
 
 def random_field(shape, nz, seed, dev, scale=1.0):
     g = torch.Generator(device=dev).manual_seed(seed)
-    f = torch.view_as_complex(torch.randn(shape + (2,), generator=g, dtype=torch.float64, device=dev)) * scale
+    r = torch.randn(shape + (2,), generator=g, dtype=torch.float64, device=dev)
+    if scale != 1.0:
+        r.mul_(scale)                            # in place: config 5 leaves room for one 14.5 GB temporary only
+    f = torch.view_as_complex(r)
     q = torch.arange(1, nz // 2, device=dev)
     f[nz - q, 0] = torch.conj(f[q, 0])          # Hermitian p = 0 column
     f[0, 0] = f[0, 0].real + 0j
@@ -78,12 +81,11 @@ def random_field(shape, nz, seed, dev, scale=1.0):
 
 
 def fullsize_names():
-    """cfg3 and cfg4 by default (about 90 s together); CHAN_TEST_FULLSIZE=cfg3 restricts the list.  cfg5 fills the
-    device with its workspace alone (146 GB), leaving no room for the seeded full-size input copies this test
-    keeps beside it: its plans are the cfg3 / cfg4 kernels at other lengths, and bench.py checks its state for
-    finiteness."""
+    """cfg3 and cfg4 by default (about 90 s together); CHAN_TEST_FULLSIZE=cfg3[,cfg4][,cfg5] restricts the list.
+    Config 5 has a memory-lean test of its own below (its 148 GB workspace leaves room for one full-size field at a
+    time) plus the cheap "cfg5-planes" / "cfg5-lines" cases."""
     env = os.environ.get("CHAN_TEST_FULLSIZE")
-    return env.split(",") if env else ["cfg3", "cfg4"]
+    return [n for n in env.split(",") if n in ("cfg3", "cfg4")] if env else ["cfg3", "cfg4"]
 
 
 @pytest.mark.parametrize("name", fullsize_names() + ["cfg5-planes"])
@@ -215,4 +217,97 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
         refs = o.velocities_vorticities()
         for fid, ref in zip((B.F_U, B.F_W, B.F_OMX, B.F_OMZ), (refs[0], refs[2], refs[3], refs[5])):
             assert rel(take_lines(ch.debug_get_field(fid), ps, ss), ref) < 1e-8, fid
+    ch.close()
+
+
+def test_config5_whole_on_sampled_lines_and_planes(B):
+    """The full 1536 x 1025 x 1152 config 5 in bench.py's launch configuration.  Memory-lean variant of the two tests
+    above: the state is staged in host memory (chan_set_state_host), every other full-size field lives on the device
+    one at a time and is regenerated from its seed when it is needed again."""
+    env = os.environ.get("CHAN_TEST_FULLSIZE")
+    if env and "cfg5" not in env.split(","):
+        pytest.skip("CHAN_TEST_FULLSIZE excludes cfg5")
+    c = inputs.config("cfg5")
+    dev = torch.device("cuda:0")
+    nz, ny = c["nz"], c["ny"]
+    shape = (nz, c["nx"] // 2, ny)
+    if torch.cuda.mem_get_info(dev)[0] < 176e9:
+        pytest.skip("config 5 needs its 148 GB workspace plus one 14.5 GB field and the filter output on the device")
+    hv, hp, ho = (torch.empty(shape, dtype=torch.complex128) for _ in range(3))
+    inputs.fluctuations(c, device=dev, zchunk=16, out=(hv, hp, ho))
+    hU, hW = torch.from_numpy(c["U"]).clone(), torch.from_numpy(c["W"]).clone()
+    torch.cuda.empty_cache()
+    ch = B.Channel(c["nx"], ny, nz, c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
+    ps, ss = sub_lattice(c)
+    sv, sphi, somy = (take_lines(t, ps, ss) for t in (hv, hp, ho))
+    base = line_oracle(c, ps, ss)
+
+    def gpu_lines(fid):
+        g = ch.debug_get_field(fid)
+        out = take_lines(g, ps, ss)
+        del g
+        return out
+
+    # ---- lines: a1-a2, then a9-a12 for the first and the last substep coefficient sets
+    ch.set_state_host(hv, hp, ho, hU, hW)
+    o = copy.deepcopy(base)
+    o.set_state(sv, sphi, somy, c["U"], c["W"])
+    for fid, ref in zip((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ), o.velocities_vorticities()):
+        assert rel(gpu_lines(fid), ref) < 1e-12, fid
+    fids = (B.F_H1, B.F_H2, B.F_H3, B.F_HV_PREV, B.F_HG_PREV)
+    for isub in (0, 2):
+        ch.set_state_host(hv, hp, ho, hU, hW)
+        Hl = []
+        for k, fid in enumerate(fids):
+            f = random_field(shape, nz, 2000 + k, dev, scale=1e2 if k < 3 else 1.0)
+            if k >= 3:
+                f[0, 0] = 0
+            Hl.append(take_lines(f, ps, ss))
+            ch.debug_set_field(fid, f)
+            del f
+            torch.cuda.empty_cache()
+        o, t = copy.deepcopy(base), copy.deepcopy(base)
+        t.__class__ = TwinOracle
+        for orc in (o, t):
+            orc.set_state(sv, sphi, somy, c["U"], c["W"])
+            orc.isub = isub
+            orc.hv_prev, orc.hg_prev = Hl[3].copy(), Hl[4].copy()
+            orc.nonlinear = lambda fields: tuple(h.copy() for h in Hl[:3])
+            orc.substep()
+        ch.debug_set_substep_index(isub)
+        ch.debug_run_stage(B.STAGE_YSOLVE)
+        e = {"v": rel(gpu_lines(B.F_V), o.v), "phi": rel(gpu_lines(B.F_PHI), o.phi), "omy": rel(gpu_lines(B.F_OMY), o.omy)}
+        ch.debug_run_stage(B.STAGE_DERIVE)
+        ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
+        prof, _ = ch.stats(B.STATS_READ)
+        e["U"] = rel(prof[0], o.U)                   # <u>(y) is the mean profile
+        fl = {"v": rel(t.v, o.v), "phi": rel(t.phi, o.phi), "omy": rel(t.omy, o.omy), "U": rel(t.U, o.U)}
+        print(f"cfg5 substep {isub}: |gpu-oracle| {e}  |twin-oracle| {fl}")
+        for k in e:
+            assert e[k] < max(TOL_SUBSTEP, 2.0 * fl[k]), (isub, k, e, fl)
+    # ---- planes: filter, statistics, nonlinear term from six seeded random fields
+    planes = sorted({0, 1, 2, ny // 3, ny // 2, 2 * ny // 3, ny - 3, ny - 2, ny - 1})
+    sampled = []
+    for k, fid in enumerate((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ)):
+        f = random_field(shape, nz, 1000 + k, dev)
+        ch.debug_set_field(fid, f)
+        sampled.append(f[:, :, planes].cpu().numpy())
+        del f
+        torch.cuda.empty_cache()
+    op = ChannelOracle(c["nx"], len(planes), nz, c["lx"], c["lz"], np.linspace(-1, 1, len(planes)), c["re"], c["dt"])
+    kxc, kzc = c["cut"]
+    got = ch.filter_store(kxc, kzc)
+    gp = got[:, planes].cpu().numpy()
+    del got
+    slots = [q % nz for q in list(range(0, kzc + 1)) + list(range(-kzc, 0))]
+    for n in range(3):
+        assert np.array_equal(gp[n], np.transpose(sampled[n][slots][:, : kxc + 1, :], (2, 0, 1))), n
+    pu, pv, pw, pox, poy, poz = (op.to_physical(f) for f in sampled)
+    for n, pr in enumerate((pu * pu, pu * pv, pu * pw, pv * pv, pv * pw, pw * pw, pox * pox + poy * poy + poz * poz)):
+        assert rel(gp[3 + n], op.to_spectral(pr, kxc, kzc)) < 1e-13, n
+    ch.debug_run_stage(B.STAGE_NONLINEAR)
+    for fid, ref_h in zip((B.F_H1, B.F_H2, B.F_H3), op.nonlinear(sampled)):
+        g = ch.debug_get_field(fid)
+        assert rel(g[:, :, planes], ref_h) < 1e-13, fid
+        del g
     ch.close()
