@@ -26,7 +26,7 @@ CHAN_HD void stc(double2* p, c2 v) { *p = make_double2(v.x, v.y); }
 // the latency of one dependent global round trip per row, not by bandwidth, at the occupancy their
 // register windows allow.
 #ifndef CHAN_PF
-#define CHAN_PF 6
+#define CHAN_PF 4
 #endif
 __device__ __forceinline__ void pf2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
