@@ -72,17 +72,24 @@ int chan_bind(chan_t* h, void* dev_workspace, size_t bytes, void* cuda_stream);
  * u, w, omega_x, omega_z (step a1).  The (0,0) mode and the z-Nyquist slot of the inputs are ignored. */
 int chan_set_state(chan_t* h, const void* dev_v, const void* dev_phi, const void* dev_omy,
                    const double* dev_U, const double* dev_W);
+/* chan_get_state leaves the handle's state, history and derived fields untouched (hence const), but it is not a
+ * pure read: it enqueues transpose kernels and copies on the bound stream like every other call. */
 int chan_get_state(const chan_t* h, void* dev_v, void* dev_phi, void* dev_omy, double* dev_U, double* dev_W);
 
-/* Same through HOST buffers (pageable or pinned): copies host->device into library scratch inside the
- * call, then behaves like the device versions; get_state_host synchronises before returning. */
+/* Same through HOST buffers (pageable or pinned).  Each field is staged through the library's scratch field, one
+ * after the other, on the bound stream; both calls SYNCHRONISE that stream before returning, so the host buffers
+ * may be reused or freed at once (set) and hold the state (get).  Neither touches any other library buffer. */
 int chan_set_state_host(chan_t* h, const void* host_v, const void* host_phi, const void* host_omy,
                         const double* host_U, const double* host_W);
 int chan_get_state_host(chan_t* h, void* host_v, void* host_phi, void* host_omy, double* host_U, double* host_W);
 
-/* One RK substep (steps a3-a12, then a1-a2 for the new state); the substep index cycles 0,1,2. */
+/* One substep of the three-substep semi-implicit low-storage Runge-Kutta scheme [34] ("A semi-implicit
+ * third-order low-storage Runge-Kutta is used for temporal integration [34]"; constants: reading R3): steps a3-a12 of
+ * DESIGN.md (nonlinear term on the dealiased grid, L80; Helmholtz/Poisson solves with the influence matrix, L100;
+ * mean mode at constant mass flux, L61), then a1-a2 for the new state.  The substep index cycles 0,1,2; the state
+ * is a physical time level only when the index is back at 0. */
 int chan_substep(chan_t* h);
-/* Three substeps; CHAN_ESTATE if called mid-step. */
+/* One full time step of PAPER.md L80 = three substeps; CHAN_ESTATE if called mid-step. */
 int chan_step(chan_t* h);
 
 /* Low-storage filter (a13): writes the ten variables u,v,w, uu,uv,uw,vv,vw,ww, om_i om_i
@@ -97,7 +104,8 @@ int chan_step_filter(chan_t* h, int kx_cut, int kz_cut, void* dev_out, size_t ou
  * CHAN_ENOSPACE if it is larger than max(one field, min(ten fields, 64 MiB)) -- use chan_filter_store then. */
 int chan_filter_store_host(chan_t* h, int kx_cut, int kz_cut, void* host_out, size_t out_bytes);
 
-/* Plane statistics (a14): flags is an OR of the values below.  ACCUMULATE adds the ten profiles
+/* Plane statistics (a14; "Regular statistics of the fully resolved flow are computed and stored
+ * on-the-fly"; the profiles are those of the ten variables of L124): flags is an OR of the values below.  ACCUMULATE adds the ten profiles
  * <u>,<v>,<w>,<uu>,<uv>,<uw>,<vv>,<vw>,<ww>,<om_i om_i> of the current state to the running sums;
  * READ copies sums[10][ny] to host_out and the sample count to *nsamples (synchronises); RESET clears. */
 #define CHAN_STATS_ACCUMULATE 1
@@ -113,11 +121,25 @@ int chan_set_pgrad(chan_t* h, double minus_dpdx); /* forcing == 1 only */
 const char* chan_strerror(int status);
 
 /* ---- tuning overrides ---------------------------------------------------------------------------
- * chan_create() reads these environment variables once (unset = the plan's own choice); they change
- * launch geometry and stage lists, never results beyond rounding:
- *   CHAN_XFUSE=4|8      radix of the x stage fused with the products      CHAN_MAXRADIX=2..12  largest stage radix (CHAN_MAXRADIX_X=2..16: x pass only)
- *   CHAN_TZ=1..16       k_x columns per z tile (power of two)              CHAN_ZTHREADS, CHAN_XTHREADS  threads per CTA
- *   CHAN_CHUNK_MB       size of the z-padded plane-chunk buffers (default 3072) */
+ * Launch geometry and stage lists; they never change results beyond rounding.  The library reads no environment
+ * variable and keeps no global state: overrides go through the handle.  chan_debug_set_tuning() must be called
+ * before chan_bind() (CHAN_ESTATE afterwards: the workspace layout depends on it); every field 0 keeps the plan's own
+ * choice; a value the plan cannot honour is CHAN_EINVAL and leaves the handle unchanged.  chan_debug_get_tuning()
+ * reports the values in effect. */
+typedef struct {
+    int xfuse;            /* 4 | 8: radix of the x stage fused with the products                                  */
+    int maxradix_z;       /* 2..12: largest radix of a z stage                                                    */
+    int maxradix_x;       /* 2..16: largest radix of an x stage in front of the fused one                          */
+    int tz;               /* k_x columns per z tile: 1, 2, 4, 8 or 16                                              */
+    int zthreads;         /* threads per CTA of the z passes, 32..256                                              */
+    int xthreads;         /* threads per CTA of the x pass, 32..256                                                */
+    int chunk_mb;         /* size of the z-padded plane-chunk buffers in MiB (default 3072)                        */
+    int planes_per_chunk; /* get only: y-planes per launch of the plane kernels that follows from chunk_mb         */
+    int plane_streams;    /* 1..3: internal streams the plane kernels of neighbouring chunks are spread over       */
+    int reserved[7];      /* must be 0                                                                             */
+} chan_tuning_t;
+int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t);
+int chan_debug_get_tuning(const chan_t* h, chan_tuning_t* out);
 
 /* ---- debug / parity / profiling hooks (run one stage on library buffers) ------------------------
  * Field ids for chan_debug_get_field / chan_debug_set_field (LINE layout, device pointers): */

@@ -24,7 +24,7 @@ EXPORTS = [
     "chan_filter_store_host", "chan_step_filter", "chan_stats", "chan_get_scalars", "chan_set_pgrad", "chan_strerror",
     "chan_debug_get_field", "chan_debug_set_field", "chan_debug_run_stage", "chan_debug_set_substep_index",
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
-    "chan_debug_profile", "chan_debug_profile_read",
+    "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
                   "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats"]
@@ -40,6 +40,13 @@ class Box(C.Structure):
 
 class Opts(C.Structure):
     _fields_ = [("lhs_halfwidth", C.c_int), ("rhs_halfwidth", C.c_int), ("forcing", C.c_int)]
+
+
+class Tuning(C.Structure):
+    """chan_tuning_t of include/chan.h (0 = the plan's own choice)."""
+    _fields_ = [("xfuse", C.c_int), ("maxradix_z", C.c_int), ("maxradix_x", C.c_int), ("tz", C.c_int), ("zthreads", C.c_int),
+                ("xthreads", C.c_int), ("chunk_mb", C.c_int), ("planes_per_chunk", C.c_int), ("plane_streams", C.c_int),
+                ("reserved", C.c_int * 7)]
 
 
 class ChanError(RuntimeError):
@@ -86,6 +93,8 @@ def load():
         "chan_debug_transpose": (i, [vp, i, vp, vp]),
         "chan_debug_profile": (i, [vp, i]),
         "chan_debug_profile_read": (i, [vp, vp, vp]),
+        "chan_debug_set_tuning": (i, [vp, C.POINTER(Tuning)]),
+        "chan_debug_get_tuning": (i, [vp, C.POINTER(Tuning)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -102,7 +111,7 @@ def _chk(status, where):
 class Channel:
     """Owner of one ``chan_t`` handle plus its torch-allocated workspace (names follow include/chan.h)."""
 
-    def __init__(self, nx, ny, nz, lx, lz, y, re_tau, dt, forcing=0, half_lhs=3, half_rhs=3):
+    def __init__(self, nx, ny, nz, lx, lz, y, re_tau, dt, forcing=0, half_lhs=3, half_rhs=3, tuning=None):
         self.lib = load()
         self.nx, self.ny, self.nz = nx, ny, nz
         y = np.ascontiguousarray(y, dtype=np.float64)
@@ -114,6 +123,22 @@ class Channel:
         _chk(self.lib.chan_create(C.byref(self.h), C.byref(grid), C.byref(box), re_tau, dt, C.byref(opts)), "chan_create")
         self.ws = None
         self.shape = (nz, nx // 2, ny)
+        if tuning:
+            self.debug_set_tuning(**tuning)
+
+    def debug_set_tuning(self, **kw):
+        """chan_debug_set_tuning (before bind): keyword = field of chan_tuning_t."""
+        t = Tuning()
+        for k, v in kw.items():
+            if k not in dict(Tuning._fields_) or k in ("reserved", "planes_per_chunk"):
+                raise KeyError(k)
+            setattr(t, k, int(v))
+        _chk(self.lib.chan_debug_set_tuning(self.h, C.byref(t)), "chan_debug_set_tuning")
+
+    def debug_get_tuning(self):
+        t = Tuning()
+        _chk(self.lib.chan_debug_get_tuning(self.h, C.byref(t)), "chan_debug_get_tuning")
+        return {k: getattr(t, k) for k, _ in Tuning._fields_ if k != "reserved"}
 
     def workspace_bytes(self):
         return int(self.lib.chan_workspace_bytes(self.h))

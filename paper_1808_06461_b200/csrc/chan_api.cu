@@ -10,7 +10,7 @@
 
 #include "../../include/chan.h"
 #include "chan_fft.cuh"
-#include "chan_fftkernels.cuh"
+#include "chan_planekernels.cuh"
 #include "chan_plan.h"
 #include "chan_ykernels.cuh"
 #include "chan_ysweeps.cuh"
@@ -46,6 +46,7 @@ struct chan {
     void (*kx3)(PlaneParams, const double2*, int, double2*, int) = nullptr;
     void (*kx7)(PlaneParams, const double2*, int, double2*, int) = nullptr;
     bool zspecial = false, xspecial = false;
+    chan_tuning_t tune = {};   // caller overrides (chan_debug_set_tuning), 0 = the plan's own choice
     // device pointers (carved)
     double2 *v, *phi, *omy, *hv, *hg, *u, *w, *ox, *oz;   // plane layout fields
     double2 *H1, *H2, *H3;                                 // alias u, w, ox
@@ -75,17 +76,16 @@ struct Carver {
 
 void choose_tiling(chan_t* h) {
     const Plan& P = h->P;
+    const chan_tuning_t& U = h->tune;
     int T = 16;
     while (T > 1 && (size_t)P.mz * T * 16 > 112 * 1024) T >>= 1;
     while (T > 1 && T > P.nxh) T >>= 1;
-    h->Tz = T;
-    h->xthreads = ((size_t)3 * P.mx * 16 > 72 * 1024) ? 256 : 128;   // <= 3 CTAs per SM: use wider CTAs
-    if (const char* e = std::getenv("CHAN_TZ")) { const int v = std::atoi(e); if (v == 1 || v == 2 || v == 4 || v == 8 || v == 16) h->Tz = v; }
-    if (const char* e = std::getenv("CHAN_ZTHREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 256) h->zthreads = v; }
-    if (const char* e = std::getenv("CHAN_XTHREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 256) h->xthreads = v; }
+    h->Tz = U.tz ? U.tz : T;
+    h->zthreads = U.zthreads ? U.zthreads : 256;
+    h->xthreads = U.xthreads ? U.xthreads : (((size_t)3 * P.mx * 16 > 72 * 1024) ? 256 : 128);   // <= 3 CTAs per SM: use wider CTAs
     const size_t per_plane = (size_t)13 * P.mz * P.nxh * 16;
-    unsigned long long budget = 3072ull << 20;    // zpad + xh: about 11 planes of config 5 per chunk (longer grids, smaller tails)
-    if (const char* e = std::getenv("CHAN_CHUNK_MB")) { const long v = std::atol(e); if (v > 0) budget = (unsigned long long)v << 20; }
+    // zpad + xh: about 11 planes of config 5 per chunk (longer grids, smaller tails)
+    const unsigned long long budget = (unsigned long long)(U.chunk_mb ? U.chunk_mb : 3072) << 20;
     long long pc = (long long)(budget / per_plane);
     if (pc < 1) pc = 1;
     if (pc > P.ny) pc = P.ny;
@@ -226,7 +226,6 @@ void pick_kernels(chan_t* h) {
 int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
     const int T = h->Tz;
     const size_t sm = (size_t)Q.mz * T * 16;
-    CK(cudaFuncSetAttribute((const void*)h->kzinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     dim3 g((Q.nxh + T - 1) / T, npl, nf);
     PB(CHAN_KC_ZFFT_INV); h->kzinv<<<g, h->zthreads, sm, h->stream>>>(Q, in, j0, npl, h->zpad, T); LAUNCHED();
     return CHAN_OK;
@@ -234,7 +233,6 @@ int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, i
 int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out, double scale, int filt, int kxc, int kzc) {
     const int T = h->Tz;
     const size_t sm = (size_t)Q.mz * T * 16;
-    CK(cudaFuncSetAttribute((const void*)h->kzfwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     dim3 g((pin + T - 1) / T, npl, nf);
     PB(filt ? CHAN_KC_ZFFT_FWD_FILTER : CHAN_KC_ZFFT_FWD);
     h->kzfwd<<<g, h->zthreads, sm, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc, T); LAUNCHED();
@@ -243,7 +241,6 @@ int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, cons
 int xprod(chan_t* h, const PlaneParams& Q, int nprod, int npl, int pout) {
     xprod_fn fn = (nprod == 3) ? h->kx3 : h->kx7;
     const size_t smx = (size_t)(nprod == 3 ? 3 : 4) * Q.mx * 16;
-    CK(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
     dim3 g(Q.mz, npl);
     PB(nprod == 3 ? CHAN_KC_XFFT_PROD : CHAN_KC_XFFT_PROD_FILTER);
     int nt = h->xthreads;
@@ -307,7 +304,6 @@ int run_ysolve(chan_t* h) {
     M.ny = P.ny; M.nm = h->nm; M.A2 = h->tab[0][1]; M.B2 = h->tab[0][2]; M.wq = h->wq; M.wm = h->wm; M.wp = h->wp;
     M.nu = P.nu; M.dt = P.dt; M.alpha = Y.alpha; M.beta = Y.beta; M.gamma = Y.gamma; M.zeta = Y.zeta; M.forcing = P.forcing;
     const size_t smm = (size_t)15 * P.ny * 8;
-    CK(cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smm));
     PB(CHAN_KC_MEAN); k_mean<<<1, 256, smm, h->stream>>>(M, h->H1, h->H3, h->U, h->W, h->H1p, h->H3p, h->scal); LAUNCHED();
     // buffers that are dead during the y-phase carry its scratch:
     // s1: zd -> z_phi -> phi_p -> zv;  oz: R_om -> z_om -> z_vab;  u, ox: factor rows (H1, H3 are consumed by SA);
@@ -323,8 +319,8 @@ int run_ysolve(chan_t* h) {
 int transpose(chan_t* h, int dir, const double2* in, double2* out) {
     const long long nm = h->nm;
     const int ny = h->P.ny;
-    const long long R = dir == 0 ? nm : ny, C = dir == 0 ? ny : nm;
-    dim3 g((unsigned)((C + 31) / 32), (unsigned)((R + 31) / 32));
+    // the mode dimension (up to 2^31 / 32 tiles) always on gridDim.x, the y dimension on gridDim.y
+    dim3 g((unsigned)((nm + 31) / 32), (unsigned)((ny + 31) / 32));
     PB(CHAN_KC_TRANSPOSE); k_transpose<<<g, 256, 0, h->stream>>>(in, out, nm, ny, dir); LAUNCHED();
     return CHAN_OK;
 }
@@ -339,6 +335,34 @@ double2* field_ptr(const chan_t* h, int f) {
     }
 }
 
+// tiling, kernel dispatch, size limits and workspace layout for the current plan and tuning overrides
+int configure(chan_t* h) {
+    if ((int)h->P.fx.radix.size() > CHAN_MAX_STAGES || (int)h->P.fz.radix.size() > CHAN_MAX_STAGES) return CHAN_EINVAL;
+    choose_tiling(h);
+    pick_kernels(h);
+    if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * h->Tz * 16 > 220 * 1024) return CHAN_EINVAL;
+    if ((size_t)15 * h->P.ny * 8 > 220 * 1024) return CHAN_EINVAL;   // mean-mode solve lives in shared memory
+    h->need = carve(h, nullptr);
+    return CHAN_OK;
+}
+
+// second half of chan_set_state: v, phi, om_y are in place (plane layout)
+int finish_set_state(chan_t* h, const double* dU, const double* dW) {
+    const Plan& P = h->P;
+    // the (0,0) mode and the z-Nyquist slot are not part of the state (reading R2)
+    for (double2* f : {h->v, h->phi, h->omy}) {
+        CK(cudaMemset2DAsync(f, (size_t)h->nm * 16, 0, 16, P.ny, h->stream));
+        CK(cudaMemset2DAsync(f + (size_t)P.nzh * P.nxh, (size_t)h->nm * 16, 0, (size_t)P.nxh * 16, P.ny, h->stream));
+    }
+    CK(cudaMemcpyAsync(h->U, dU, (size_t)P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->W, dW, (size_t)P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemsetAsync(h->hv, 0, h->F, h->stream)); CK(cudaMemsetAsync(h->hg, 0, h->F, h->stream));
+    CK(cudaMemsetAsync(h->H1p, 0, (size_t)P.ny * 8, h->stream)); CK(cudaMemsetAsync(h->H3p, 0, (size_t)P.ny * 8, h->stream));
+    PB(CHAN_KC_MEAN); k_flux<<<1, 32, 0, h->stream>>>(P.ny, h->wq, h->U, h->scal); LAUNCHED();
+    h->isub = 0; h->have_state = true;
+    return run_derive(h);
+}
+
 }  // namespace
 
 extern "C" {
@@ -351,15 +375,42 @@ int chan_create(chan_t** out, const chan_grid_t* grid, const chan_box_t* box, do
     const int hl = opts ? opts->lhs_halfwidth : 3, hr = opts ? opts->rhs_halfwidth : 3, fo = opts ? opts->forcing : 0;
     int rc = build_plan(h->P, grid->nx, grid->ny, grid->nz, box->lx, box->lz, box->y, re_tau, dt, hl ? hl : 3, hr ? hr : 3, fo);
     if (rc != CHAN_OK) { delete h; return rc; }
-    if ((int)h->P.fx.radix.size() > CHAN_MAX_STAGES || (int)h->P.fz.radix.size() > CHAN_MAX_STAGES) { delete h; return CHAN_EINVAL; }
     h->nm = (long long)h->P.nz * h->P.nxh;
     h->F = (size_t)h->nm * h->P.ny * 16;
-    choose_tiling(h);
-    pick_kernels(h);
-    if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * 16 > 220 * 1024) { delete h; return CHAN_EINVAL; }
-    if ((size_t)15 * h->P.ny * 8 > 220 * 1024) { delete h; return CHAN_EINVAL; }   // mean-mode solve lives in shared memory
-    h->need = carve(h, nullptr);
+    if ((rc = configure(h)) != CHAN_OK) { delete h; return rc; }
     *out = h;
+    return CHAN_OK;
+}
+
+int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t) {
+    if (!h || !t) return CHAN_EINVAL;
+    if (h->bound) return CHAN_ESTATE;
+    for (int r : t->reserved) if (r) return CHAN_EINVAL;
+    auto pow2 = [](int v) { return v == 1 || v == 2 || v == 4 || v == 8 || v == 16; };
+    if ((t->xfuse && t->xfuse != 4 && t->xfuse != 8) || (t->maxradix_z && (t->maxradix_z < 2 || t->maxradix_z > 12)) ||
+        (t->maxradix_x && (t->maxradix_x < 2 || t->maxradix_x > 16)) || (t->tz && !pow2(t->tz)) ||
+        (t->zthreads && (t->zthreads < 32 || t->zthreads > 256)) || (t->xthreads && (t->xthreads < 32 || t->xthreads > 256)) ||
+        t->chunk_mb < 0 || t->plane_streams < 0 || t->plane_streams > 3)
+        return CHAN_EINVAL;
+    const chan_tuning_t old = h->tune;
+    const FftPlan ofx = h->P.fx, ofz = h->P.fz;
+    h->tune = *t;
+    int rc = plan_ffts(h->P, t->xfuse, t->maxradix_z, t->maxradix_x);
+    if (rc == CHAN_OK) rc = configure(h);
+    if (rc != CHAN_OK) { h->tune = old; h->P.fx = ofx; h->P.fz = ofz; configure(h); }
+    return rc;
+}
+
+int chan_debug_get_tuning(const chan_t* h, chan_tuning_t* out) {
+    if (!h || !out) return CHAN_EINVAL;
+    *out = chan_tuning_t{};
+    out->xfuse = h->P.fx.radix.back();
+    for (int r : h->P.fz.radix) out->maxradix_z = r > out->maxradix_z ? r : out->maxradix_z;
+    for (size_t k = 0; k + 1 < h->P.fx.radix.size(); ++k) out->maxradix_x = h->P.fx.radix[k] > out->maxradix_x ? h->P.fx.radix[k] : out->maxradix_x;
+    out->tz = h->Tz; out->zthreads = h->zthreads; out->xthreads = h->xthreads;
+    out->chunk_mb = h->tune.chunk_mb ? h->tune.chunk_mb : 3072;
+    out->planes_per_chunk = h->pc;
+    out->plane_streams = h->tune.plane_streams ? h->tune.plane_streams : 1;
     return CHAN_OK;
 }
 
@@ -391,6 +442,12 @@ int chan_bind(chan_t* h, void* dev_workspace, size_t bytes, void* cuda_stream) {
     CK(upl(h->wq, P.wq.data(), P.wq.size() * 8));
     CK(upl(h->twx, P.fx.tw.data(), P.fx.tw.size() * 8)); CK(upl(h->twz, P.fz.tw.data(), P.fz.tw.size() * 8));
     CK(cudaStreamSynchronize(h->stream));   // the host vectors may not outlive the copies otherwise
+    // dynamic shared memory of the kernels this handle dispatches to, once (not per launch)
+    CK(cudaFuncSetAttribute((const void*)h->kzinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P.mz * h->Tz * 16)));
+    CK(cudaFuncSetAttribute((const void*)h->kzfwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P.mz * h->Tz * 16)));
+    CK(cudaFuncSetAttribute((const void*)h->kx3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)3 * P.mx * 16)));
+    CK(cudaFuncSetAttribute((const void*)h->kx7, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)4 * P.mx * 16)));
+    CK(cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)15 * P.ny * 8)));
     h->bound = true; h->have_state = false; h->isub = 0; h->nsamples = 0;
     return CHAN_OK;
 }
@@ -402,19 +459,7 @@ int chan_set_state(chan_t* h, const void* dv, const void* dphi, const void* domy
     if ((rc = transpose(h, 0, (const double2*)dv, h->v))) return rc;
     if ((rc = transpose(h, 0, (const double2*)dphi, h->phi))) return rc;
     if ((rc = transpose(h, 0, (const double2*)domy, h->omy))) return rc;
-    const Plan& P = h->P;
-    // the (0,0) mode and the z-Nyquist slot are not part of the state (reading R2)
-    for (double2* f : {h->v, h->phi, h->omy}) {
-        CK(cudaMemset2DAsync(f, (size_t)h->nm * 16, 0, 16, P.ny, h->stream));
-        CK(cudaMemset2DAsync(f + (size_t)P.nzh * P.nxh, (size_t)h->nm * 16, 0, (size_t)P.nxh * 16, P.ny, h->stream));
-    }
-    CK(cudaMemcpyAsync(h->U, dU, (size_t)P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
-    CK(cudaMemcpyAsync(h->W, dW, (size_t)P.ny * 8, cudaMemcpyDeviceToDevice, h->stream));
-    CK(cudaMemsetAsync(h->hv, 0, h->F, h->stream)); CK(cudaMemsetAsync(h->hg, 0, h->F, h->stream));
-    CK(cudaMemsetAsync(h->H1p, 0, (size_t)P.ny * 8, h->stream)); CK(cudaMemsetAsync(h->H3p, 0, (size_t)P.ny * 8, h->stream));
-    PB(CHAN_KC_MEAN); k_flux<<<1, 32, 0, h->stream>>>(P.ny, h->wq, h->U, h->scal); LAUNCHED();
-    h->isub = 0; h->have_state = true;
-    return run_derive(h);
+    return finish_set_state(h, dU, dW);
 }
 
 int chan_get_state(const chan_t* hc, void* dv, void* dphi, void* domy, double* dU, double* dW) {
@@ -430,30 +475,37 @@ int chan_get_state(const chan_t* hc, void* dv, void* dphi, void* domy, double* d
     return CHAN_OK;
 }
 
+// Host state in: each field goes host -> s1 (scratch field, idle between substeps) -> transposed into place, one after the
+// other on the bound stream; the tail of chan_set_state (Nyquist/mean slots, history, mass flux, a1) follows.
 int chan_set_state_host(chan_t* h, const void* hv, const void* hphi, const void* homy, const double* hU, const double* hW) {
     if (!h || !hv || !hphi || !homy || !hU || !hW) return CHAN_EINVAL;
     if (!h->bound) return CHAN_ESTATE;
-    // stage the three fields in the derived-field buffers (rebuilt by set_state), the profiles in meanwork
-    double2* st[3] = {h->u, h->w, h->ox};
+    double2* dst[3] = {h->v, h->phi, h->omy};
     const void* src[3] = {hv, hphi, homy};
-    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(st[k], src[k], h->F, cudaMemcpyHostToDevice, h->stream));
+    int rc;
+    for (int k = 0; k < 3; ++k) {
+        CK(cudaMemcpyAsync(h->s1, src[k], h->F, cudaMemcpyHostToDevice, h->stream));
+        if ((rc = transpose(h, 0, h->s1, dst[k]))) return rc;
+    }
     CK(cudaMemcpyAsync(h->meanwork, hU, (size_t)h->P.ny * 8, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyAsync(h->meanwork + h->P.ny, hW, (size_t)h->P.ny * 8, cudaMemcpyHostToDevice, h->stream));
-    return chan_set_state(h, st[0], st[1], st[2], h->meanwork, h->meanwork + h->P.ny);
+    if ((rc = finish_set_state(h, h->meanwork, h->meanwork + h->P.ny))) return rc;
+    CK(cudaStreamSynchronize(h->stream));     // the host buffers are the caller's again when this returns (chan.h)
+    return CHAN_OK;
 }
 
 int chan_get_state_host(chan_t* h, void* hv, void* hphi, void* homy, double* hU, double* hW) {
     if (!h || !hv || !hphi || !homy || !hU || !hW) return CHAN_EINVAL;
     if (!h->bound || !h->have_state) return CHAN_ESTATE;
-    // staged in the derived-field buffers u, w, om_x, which are rebuilt (step a1) after the copies are queued
-    double2* st[3] = {h->u, h->w, h->ox};
-    int rc = chan_get_state(h, st[0], st[1], st[2], h->meanwork, h->meanwork + h->P.ny);
-    if (rc) return rc;
+    double2* src[3] = {h->v, h->phi, h->omy};
     void* dst[3] = {hv, hphi, homy};
-    for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(dst[k], st[k], h->F, cudaMemcpyDeviceToHost, h->stream));
-    CK(cudaMemcpyAsync(hU, h->meanwork, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
-    CK(cudaMemcpyAsync(hW, h->meanwork + h->P.ny, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
-    if ((rc = run_derive(h))) return rc;
+    int rc;
+    for (int k = 0; k < 3; ++k) {
+        if ((rc = transpose(h, 1, src[k], h->s1))) return rc;
+        CK(cudaMemcpyAsync(dst[k], h->s1, h->F, cudaMemcpyDeviceToHost, h->stream));
+    }
+    CK(cudaMemcpyAsync(hU, h->U, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaMemcpyAsync(hW, h->W, (size_t)h->P.ny * 8, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return CHAN_OK;
 }

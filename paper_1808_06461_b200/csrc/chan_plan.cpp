@@ -235,6 +235,28 @@ bool make_fft_plan(int n, int fused_last, int maxr, FftPlan& F) {
 
 }  // namespace
 
+// Stage lists of the two transform lengths.  xfuse: 4 | 8 = radix of the x stage fused with the products (0: the one
+// that gives the shorter stage list, then the one without radix-12 stages, then 4: lighter fused stage);
+// maxr: largest radix of a z stage (0: 12); maxrx: largest radix of an x stage (0: 16 -- two shared-memory stages in
+// front of the fused one at 1536 points).
+int plan_ffts(Plan& P, int xfuse, int maxr, int maxrx) {
+    if (maxr < 2) maxr = 12;
+    if (maxrx < 2) maxrx = 16;
+    int fuse = 4;
+    if (xfuse == 4 || xfuse == 8) fuse = xfuse;
+    else {
+        FftPlan f4, f8;
+        auto key = [](const FftPlan& f) {
+            int big = 0;
+            for (int r : f.radix) big += (r == 12) + 3 * (r > 12);
+            return (int)f.radix.size() * 100 + big;
+        };
+        if (make_fft_plan(P.mx, 4, maxrx, f4) && make_fft_plan(P.mx, 8, maxrx, f8) && key(f8) < key(f4)) fuse = 8;
+    }
+    if (!make_fft_plan(P.mx, fuse, maxrx, P.fx) || !make_fft_plan(P.mz, 0, maxr, P.fz)) return CHAN_EINVAL;
+    return CHAN_OK;
+}
+
 int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const double* y, double re_tau, double dt,
                int half_lhs, int half_rhs, int forcing) {
     if (nx < 4 || nz < 4 || (nx & 1) || (nz & 1) || ny < 8 || !y) return CHAN_EINVAL;
@@ -246,29 +268,8 @@ int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const doub
     P.lx = lx; P.lz = lz; P.nu = 1.0 / re_tau; P.dt = dt;
     P.half_lhs = half_lhs; P.half_rhs = half_rhs; P.forcing = forcing;
     P.y.assign(y, y + ny);
-    // x: the last stage is fused with the products and needs the 8-aligned swizzle of chan_fft.cuh
-    if (P.mx % 8) return CHAN_EINVAL;
-    const char* ef = std::getenv("CHAN_XFUSE");
-    const char* er = std::getenv("CHAN_MAXRADIX");
-    const int maxr = (er && std::atoi(er) >= 2) ? std::atoi(er) : 12;
-    // the x pass may use radix 16 (two shared-memory stages in front of the fused one at 1536 points; radix 18, which
-    // would do the same at 2304 points, was measured slower: it spills ~400 bytes under the 128-register cap);
-    // the z passes stay at 12
-    const char* erx = std::getenv("CHAN_MAXRADIX_X");
-    const int maxrx = er ? maxr : ((erx && std::atoi(erx) >= 2) ? std::atoi(erx) : 16);
-    int fuse = 4;
-    if (ef) fuse = (std::atoi(ef) == 8) ? 8 : 4;
-    else {   // the fused radix (4 or 8) that gives the shorter stage list, then the one without radix-12 stages
-             // (they spill under the 128-register cap), then 4 (lighter fused stage)
-        FftPlan f4, f8;
-        auto key = [](const FftPlan& f) {
-            int big = 0;
-            for (int r : f.radix) big += (r == 12) + 3 * (r > 12);
-            return (int)f.radix.size() * 100 + big;
-        };
-        if (make_fft_plan(P.mx, 4, maxrx, f4) && make_fft_plan(P.mx, 8, maxrx, f8) && key(f8) < key(f4)) fuse = 8;
-    }
-    if (!make_fft_plan(P.mx, fuse, maxrx, P.fx) || !make_fft_plan(P.mz, 0, maxr, P.fz)) return CHAN_EINVAL;
+    if (P.mx % 8) return CHAN_EINVAL;   // x: the last stage is fused with the products and needs the 8-aligned swizzle of chan_fft.cuh
+    if (int rc = plan_ffts(P, 0, 0, 0)) return rc;
 
     // RK3 constants of [34] (reading R3)
     const double al[3] = {29.0 / 96.0, -3.0 / 40.0, 1.0 / 6.0}, be[3] = {37.0 / 160.0, 5.0 / 24.0, 1.0 / 6.0};

@@ -41,6 +41,10 @@ struct Plan {
     double rk_alpha[3], rk_beta[3], rk_gamma[3], rk_zeta[3];
 };
 
+// Stage lists of the x and z transforms (0 = the planner's own choice, see chan_plan.cpp); build_plan calls it with
+// zeros, chan_debug_set_tuning() again with the caller's overrides.  Returns 0 or CHAN_EINVAL.
+int plan_ffts(Plan& P, int xfuse, int maxradix_z, int maxradix_x);
+
 // Returns 0 or a CHAN_E* status.
 int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const double* y, double re_tau, double dt,
                int half_lhs, int half_rhs, int forcing);

@@ -75,7 +75,8 @@ __global__ void __launch_bounds__(256) k_transpose(const double2* __restrict__ i
     __shared__ double2 tile[32][33];
     // in is [R][C] -> out [C][R]
     const long long R = dir == 0 ? nm : ny, C = dir == 0 ? ny : nm;
-    const long long c0 = (long long)blockIdx.x * 32, r0 = (long long)blockIdx.y * 32;
+    // the mode dimension is tiled by blockIdx.x in both directions (gridDim.y is limited to 65535 tiles)
+    const long long c0 = (long long)(dir == 0 ? blockIdx.y : blockIdx.x) * 32, r0 = (long long)(dir == 0 ? blockIdx.x : blockIdx.y) * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // 32 x 8
     for (int k = ty; k < 32; k += 8) {
         const long long r = r0 + k, c = c0 + tx;

@@ -354,6 +354,9 @@ __global__ void __launch_bounds__(YNT) k_sc(YParams P, double2* facA, double2* f
                     *wpart(zom_zvab, oc, part) = zab;
                     if (part == 0) facA[oc] = make_double2(f.x, f.y); else facB[oc] = make_double2(f.z, f.w);
                 }
+                // both lanes of a mode read facA/facB at row jj+1 while only one of them writes each at row jj-3:
+                // keep the pair (and so the four-row gap) in step without relying on implicit warp lockstep
+                __syncwarp();
                 ol += nm;
             }
         });

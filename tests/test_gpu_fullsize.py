@@ -5,10 +5,13 @@ the wall-normal stages act on each (kx,kz) line independently and the wall-paral
 independently.  So the full-size GPU result is compared with the oracle on SAMPLED lines and planes:
 
 * lines: a small ChannelOracle on the same mesh whose wavenumber tables are overwritten with those of a
-  sub-lattice {p} x {z slot} of the big grid (including the mean mode and the z-Nyquist slot) computes exactly
-  those lines of the big problem;
-* planes: a ChannelOracle with the full nx, nz but only the sampled planes runs the padded transforms, the
-  products, the filter products and the statistics of those planes.
+  64 x 64 sub-lattice {p} x {z slot} of the big grid (4096 lines, including the mean mode and the z-Nyquist slot)
+  computes exactly those lines of the big problem; the long-double yardstick (oracle/channel_hp.py) runs on a
+  16 x 16 sub-lattice of those and gives the oracle's own rounding error, which sets the gate where it exceeds
+  north_star's 1e-11 (DESIGN.md section 7);
+* planes: a ChannelOracle with the full nx, nz runs the padded transforms, the products, the filter products and
+  the statistics of 64 sampled planes (in batches of 8), among them both sides of the first, a middle and the last
+  plane-chunk seam of the launch configuration (chan_debug_get_tuning: planes_per_chunk).
 
 All inputs are seeded; the oracle receives copies of the very arrays handed to the library.
 """
@@ -22,7 +25,7 @@ import torch
 import __graft_entry__ as entry
 from oracle.channel import ChannelOracle
 from paper_1808_06461_b200 import inputs
-from test_gpu_parity import TwinOracle, rel
+from test_gpu_parity import K_FLOOR, K_LINE, line_rel, make_hp, rel
 
 pytestmark = pytest.mark.gpu
 
@@ -38,7 +41,7 @@ def B():
     return binding
 
 
-def sub_lattice(c, npx=8, nsz=8):
+def sub_lattice(c, npx=64, nsz=64):
     """Index lists (p, z slot) of the sampled lines; entry [0] of each is 0 (mean mode) and the middle z entry is
     the Nyquist slot, so the small oracle's special cases coincide with the big grid's."""
     nxh, nz = c["nx"] // 2, c["nz"]
@@ -58,6 +61,154 @@ def line_oracle(c, ps, ss, cls=ChannelOracle):
     o.kx, o.kz = kx[ps].copy(), kz[ss].copy()
     o.k2 = o.kz[:, None] ** 2 + o.kx[None, :] ** 2
     return o
+
+
+HP_STRIDE = 4      # the long-double yardstick runs on every 4th p and z slot of the sub-lattice (16 x 16 lines)
+
+
+def sub_oracle(base, ps, ss, ip, iz):
+    """The oracle restricted to the lines (ss[iz], ps[ip]) of `base` (which already carries the sampled wavenumbers):
+    same tables (built once in exact rationals), fresh state.  iz must keep 0 first and the Nyquist slot in the middle."""
+    o = copy.copy(base)
+    o.nx, o.nz = 2 * len(ip), len(iz)
+    o.mx, o.mz = 3 * o.nx // 2, 3 * o.nz // 2
+    o.kx, o.kz = base.kx[ip].copy(), base.kz[iz].copy()
+    o.k2 = o.kz[:, None] ** 2 + o.kx[None, :] ** 2
+    shp = (o.nz, o.nx // 2, o.ny)
+    o.v, o.phi, o.omy, o.hv_prev, o.hg_prev = (np.zeros(shp, complex) for _ in range(5))
+    o.U, o.W, o.H1m_prev, o.H3m_prev = (np.zeros(o.ny) for _ in range(4))
+    return o
+
+
+def hp_indices(ps, ss):
+    ip, iz = np.arange(0, ps.size, HP_STRIDE), np.arange(0, ss.size, HP_STRIDE)
+    assert ip[0] == 0 and iz[0] == 0 and iz[iz.size // 2] == ss.size // 2      # mean mode and Nyquist slot stay in place
+    return ip, iz
+
+
+def ysolve_reference(base, ps, ss, state, Hl, isub, c):
+    """Oracle on all sampled lines and long-double yardstick on the 16 x 16 subset, for one substep coefficient set from
+    seeded H and history.  Returns (oracle, subset oracle, yardstick, subset index arrays)."""
+    sv, sphi, somy = state
+    o = copy.deepcopy(base)
+    o.set_state(sv, sphi, somy, c["U"], c["W"])
+    o.isub = isub
+    o.hv_prev, o.hg_prev = Hl[3].copy(), Hl[4].copy()
+    o.nonlinear = lambda fields: tuple(h.copy() for h in Hl[:3])
+    o.substep()
+    ip, iz = hp_indices(ps, ss)
+    pick = lambda a: a[np.ix_(iz, ip)]
+    os_ = sub_oracle(base, ps, ss, ip, iz)
+    hp = make_hp(os_)
+    for orc in (os_, hp):
+        orc.set_state(pick(sv), pick(sphi), pick(somy), c["U"], c["W"])
+        orc.isub = isub
+        orc.hv_prev, orc.hg_prev = pick(Hl[3]).astype(orc.v.dtype), pick(Hl[4]).astype(orc.v.dtype)
+    os_.nonlinear = lambda fields: tuple(pick(h).copy() for h in Hl[:3])
+    hp.nonlinear_override = lambda fields: tuple(pick(h) for h in Hl[:3])
+    os_.substep()
+    hp.substep()
+    # the subset oracle is the big one restricted (same arithmetic per line): bit for bit
+    assert np.array_equal(os_.phi, pick(o.phi)) and np.array_equal(os_.v, pick(o.v))
+    return o, os_, hp, (ip, iz)
+
+
+def gate_ysolve(name, isub, gpu, o, os_, hp, sub):
+    """gpu = (v, phi, om_y lines [64][64][ny], U).  Whole-sample relative L2 and per-line gates."""
+    ip, iz = sub
+    pick = lambda a: a[np.ix_(iz, ip)]
+    e, fl, eh = {}, {}, {}
+    for k, g in zip(("v", "phi", "omy"), gpu[:3]):
+        ref = getattr(o, k)
+        hpk = np.asarray(getattr(hp, k)).astype(complex)
+        e[k] = rel(g, ref)
+        fl[k] = rel(getattr(os_, k), hpk)                 # oracle's own rounding error (16 x 16 lines)
+        eh[k] = rel(pick(g), hpk)                         # kernel's rounding error on the same lines
+    e["U"], fl["U"], eh["U"] = rel(gpu[3], o.U), rel(os_.U, np.asarray(hp.U).astype(float)), rel(gpu[3], np.asarray(hp.U).astype(float))
+    print(f"{name} substep set {isub}: |gpu-oracle| {e}  |oracle-hp| {fl}  |gpu-hp| {eh}")
+    for k in e:
+        lim = max(TOL_SUBSTEP, K_FLOOR * fl[k])
+        assert e[k] < lim and eh[k] < lim, (isub, k, e, fl, eh)
+    assert max(e["v"], e["U"]) < TOL_SUBSTEP, (isub, e)    # the primitive unknowns meet north_star outright
+    # per line: all 4096 against the oracle, bound = the worst oracle rounding error among the yardstick's lines
+    for k, g in zip(("v", "phi", "omy"), gpu[:3]):
+        ref = getattr(o, k)
+        el = line_rel(g, ref)
+        fworst = float(line_rel(np.asarray(getattr(hp, k)).astype(complex), getattr(os_, k)).max())
+        assert el.max() < max(TOL_SUBSTEP, K_LINE * fworst), (isub, k, "line", np.unravel_index(np.argmax(el), el.shape), float(el.max()), fworst)
+
+
+def sample_planes(ny, pc, n=64):
+    """n plane indices: the walls and their neighbours, both sides of the first, a middle and the last chunk seam
+    (chunks are [k pc, (k+1) pc)), the rest spread over y."""
+    must = {0, 1, 2, ny - 3, ny - 2, ny - 1, ny // 2}
+    nch = (ny + pc - 1) // pc
+    for k in {1, nch // 2, nch - 1}:
+        if 0 < k < nch:
+            must |= {k * pc - 1, k * pc}
+    must = {j for j in must if 0 <= j < ny}
+    rng = np.random.default_rng(17)
+    rest = rng.permutation(np.setdiff1d(np.arange(ny), sorted(must)))[: max(0, min(n, ny) - len(must))]
+    return sorted(must | set(int(j) for j in rest))
+
+
+def planes_check(B, ch, c, planes, sampled, nonlinear=True):
+    """a13, a14, a3-a8 on the sampled planes against the oracle, in batches of 8 planes.  sampled: six numpy arrays
+    [nz][nxh][len(planes)] = the seeded fields on those planes."""
+    nz = c["nz"]
+    kxc, kzc = c["cut"]
+    got = ch.filter_store(kxc, kzc)
+    gp = got[:, planes].cpu().numpy()
+    del got
+    slots = [q % nz for q in list(range(0, kzc + 1)) + list(range(-kzc, 0))]
+    for n in range(3):
+        assert np.array_equal(gp[n], np.transpose(sampled[n][slots][:, : kxc + 1, :], (2, 0, 1))), n
+    ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
+    prof, ns = ch.stats(B.STATS_READ)
+    assert ns == 1
+    wp = np.full(c["nx"] // 2, 2.0)
+    wp[0] = 1.0
+    mean = lambda a, b: np.einsum("p,qpy->y", wp, (a * np.conj(b)).real)
+    u, v, w, ox, oy, oz = sampled
+    ref = [u[0, 0].real, v[0, 0].real, w[0, 0].real, mean(u, u), mean(u, v), mean(u, w), mean(v, v), mean(v, w), mean(w, w),
+           mean(ox, ox) + mean(oy, oy) + mean(oz, oz)]
+    for n in range(10):
+        assert np.abs(prof[n][planes] - ref[n]).max() < 1e-12 * max(1.0, np.abs(ref[n]).max()), n
+    for n in range(3, 10):   # second-order consistency on the GPU side: (0,0) mode of the stored products == statistics
+        assert np.abs(gp[n][:, 0, 0].real - prof[n][planes]).max() < 1e-11 * np.abs(prof[n]).max()
+    H = None
+    if nonlinear:
+        ch.debug_run_stage(B.STAGE_NONLINEAR)
+        H = []
+        for fid in (B.F_H1, B.F_H2, B.F_H3):
+            g = ch.debug_get_field(fid)
+            assert not bool(g[nz // 2].any())
+            H.append(g[:, :, planes].cpu().numpy())
+            del g
+    nb = 8
+    o = ChannelOracle(c["nx"], nb, nz, c["lx"], c["lz"], np.linspace(-1, 1, nb), c["re"], c["dt"])
+    worst = 0.0
+    for b0 in range(0, len(planes), nb):
+        sl = slice(b0, min(b0 + nb, len(planes)))
+        cnt = sl.stop - sl.start
+        batch = []
+        for f in sampled:                       # pad the last batch with zero planes: the oracle is built for nb planes
+            a = np.zeros(f.shape[:2] + (nb,), complex)
+            a[:, :, :cnt] = f[:, :, sl]
+            batch.append(a)
+        pu, pv, pw, pox, poy, poz = (o.to_physical(f) for f in batch)
+        prods = (pu * pu, pu * pv, pu * pw, pv * pv, pv * pw, pw * pw, pox * pox + poy * poy + poz * poz)
+        for n, pr in enumerate(prods):
+            r = rel(gp[3 + n][sl], o.to_spectral(pr, kxc, kzc)[:cnt])
+            worst = max(worst, r)
+            assert r < 1e-13, (n, b0)
+        if nonlinear:
+            refs = (o.to_spectral(pv * poz - pw * poy), o.to_spectral(pw * pox - pu * poz), o.to_spectral(pu * poy - pv * pox))
+            for g, ref_h in zip(H, refs):
+                r = rel(g[:, :, sl], ref_h[:, :, :cnt])
+                worst = max(worst, r)
+                assert r < 1e-13, b0
+    print(f"planes {len(planes)} (seams included): worst relative L2 of a batch of 8 planes {worst:.2e}")
 
 
 def take_lines(t, ps, ss):
@@ -90,13 +241,20 @@ def fullsize_names():
 
 @pytest.mark.parametrize("name", fullsize_names() + ["cfg5-planes"])
 def test_fullsize_planes_filter_stats(B, name):
-    """a3-a8, a13, a14 at full size on sampled planes, from six seeded random Hermitian fields.
-    "cfg5-planes": the 1536 x 1152 wall-parallel grid of config 5 (its transform plans and tiles) on 9 planes."""
-    c = inputs.config("cfg5", ny=9) if name == "cfg5-planes" else inputs.config(name)
+    """a3-a8, a13, a14 at full size on 64 sampled planes (chunk seams included), from six seeded random Hermitian
+    fields.  "cfg5-planes": the 1536 x 1152 wall-parallel grid of config 5 (its transform plans and tiles) on 72 planes
+    with the plane chunks cut down to 11 planes as in the full config 5, so that the seams exist."""
+    if name == "cfg5-planes":
+        c = inputs.config("cfg5", ny=72)
+        tuning = None            # 3 GB chunks = 11 planes of this plane size, as in the full config
+    else:
+        c, tuning = inputs.config(name), None
     dev = torch.device("cuda:0")
-    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
+    ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"], tuning=tuning).bind(dev)
     nz, ny = c["nz"], c["ny"]
-    planes = sorted({0, 1, 2, ny // 3, ny // 2, 2 * ny // 3, ny - 3, ny - 2, ny - 1})    # the oracle wants at least 8 mesh points
+    pc = ch.debug_get_tuning()["planes_per_chunk"]
+    planes = sample_planes(ny, pc)
+    assert len(planes) == min(64, ny) and (pc >= ny or {pc - 1, pc} <= set(planes))
     fids = (B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ)
     z = torch.zeros(ch.shape, dtype=torch.complex128, device=dev)
     ch.set_state(z, z, z, c["U"], c["W"])       # the filter and the statistics want a state; the six fields are overwritten below
@@ -109,68 +267,34 @@ def test_fullsize_planes_filter_stats(B, name):
         sampled.append(f[:, :, planes].cpu().numpy())
         del f
     torch.cuda.empty_cache()
-    o = ChannelOracle(c["nx"], len(planes), nz, c["lx"], c["lz"], np.linspace(-1, 1, len(planes)), c["re"], c["dt"])
-    # filter (a13): bit-exact mode selection, products on the dealiased grid
-    kxc, kzc = c["cut"]
-    got = ch.filter_store(kxc, kzc)
-    gp = got[:, planes].cpu().numpy()
-    del got
-    slots = [q % nz for q in list(range(0, kzc + 1)) + list(range(-kzc, 0))]
-    for n in range(3):
-        assert np.array_equal(gp[n], np.transpose(sampled[n][slots][:, : kxc + 1, :], (2, 0, 1))), n
-    pu, pv, pw, pox, poy, poz = (o.to_physical(f) for f in sampled)
-    prods = (pu * pu, pu * pv, pu * pw, pv * pv, pv * pw, pw * pw, pox * pox + poy * poy + poz * poz)
-    for n, pr in enumerate(prods):
-        assert rel(gp[3 + n], o.to_spectral(pr, kxc, kzc)) < 1e-13, n
-    # statistics (a14)
-    ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
-    prof, ns = ch.stats(B.STATS_READ)
-    assert ns == 1
-    wp = np.full(c["nx"] // 2, 2.0)
-    wp[0] = 1.0
-    mean = lambda a, b: np.einsum("p,qpy->y", wp, (a * np.conj(b)).real)
-    u, v, w, ox, oy, oz = sampled
-    ref = [u[0, 0].real, v[0, 0].real, w[0, 0].real, mean(u, u), mean(u, v), mean(u, w), mean(v, v), mean(v, w), mean(w, w),
-           mean(ox, ox) + mean(oy, oy) + mean(oz, oz)]
-    for n in range(10):
-        assert np.abs(prof[n][planes] - ref[n]).max() < 1e-12 * max(1.0, np.abs(ref[n]).max()), n
-    # second-order consistency on the GPU side: (0,0) mode of the stored products == plane statistics
-    for n in range(3, 10):
-        assert np.abs(gp[n][:, 0, 0].real - prof[n][planes]).max() < 1e-11 * np.abs(prof[n]).max()
-    # nonlinear term (a3-a8)
-    ch.debug_run_stage(B.STAGE_NONLINEAR)
-    H = o.nonlinear(sampled)
-    for fid, ref_h in zip((B.F_H1, B.F_H2, B.F_H3), H):
-        g = ch.debug_get_field(fid)
-        assert rel(g[:, :, planes], ref_h) < 1e-13, fid
-        assert not bool(g[nz // 2].any())
-        del g
+    planes_check(B, ch, c, planes, sampled)
     ch.close()
 
 
 @pytest.mark.parametrize("name", fullsize_names() + ["cfg5-lines"])
 def test_fullsize_lines_derive_and_ysolve(B, name):
-    """a1-a2 and a9-a12 at full size on a sub-lattice of lines, for the three substep coefficient sets.
-    "cfg5-lines": the 1025-point mesh, Re and dt of config 5 on a 32 x 16 sub-box with the same dx, dz (the same
-    range of wavenumbers and Helmholtz parameters, the full line length)."""
+    """a1-a2 and a9-a12 at full size on 4096 sampled lines, for the three substep coefficient sets.
+    "cfg5-lines": the 1025-point mesh, Re and dt of config 5 on a 128 x 64 sub-box with the same dx, dz (the same
+    range of wavenumbers and Helmholtz parameters, the full line length, every line sampled)."""
     if name == "cfg5-lines":
         c5 = inputs.CONFIGS["cfg5"]
-        c = inputs.config("cfg5", nx=32, nz=16, lx=c5["lx"] * 32 / c5["nx"], lz=c5["lz"] * 16 / c5["nz"])
+        c = inputs.config("cfg5", nx=128, nz=64, lx=c5["lx"] * 128 / c5["nx"], lz=c5["lz"] * 64 / c5["nz"])
+        ps, ss = np.arange(64), np.arange(64)
     else:
         c = inputs.config(name)
+        ps, ss = sub_lattice(c)
     dev = torch.device("cuda:0")
     ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
     nz = c["nz"]
-    ps, ss = sub_lattice(c)
     v, phi, omy = inputs.fluctuations(c, device=dev, zchunk=64)
-    sv, sphi, somy = (take_lines(t, ps, ss) for t in (v, phi, omy))
+    state = tuple(take_lines(t, ps, ss) for t in (v, phi, omy))
     ch.set_state(v, phi, omy, c["U"], c["W"])
     del v, phi, omy
     ch._keep = None
     torch.cuda.empty_cache()
     base = line_oracle(c, ps, ss)
     o = copy.deepcopy(base)
-    o.set_state(sv, sphi, somy, c["U"], c["W"])
+    o.set_state(*state, c["U"], c["W"])
     # a1-a2
     refs = o.velocities_vorticities()
     for fid, ref in zip((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ), refs):
@@ -186,14 +310,7 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
         Hl.append(take_lines(f, ps, ss))
         Hs.append(f)
     for isub in range(3):
-        o, t = copy.deepcopy(base), copy.deepcopy(base)     # fresh: no mean-flow history (the exact-rational tables are built once)
-        t.__class__ = TwinOracle
-        for orc in (o, t):
-            orc.set_state(sv, sphi, somy, c["U"], c["W"])
-            orc.isub = isub
-            orc.hv_prev, orc.hg_prev = Hl[3].copy(), Hl[4].copy()
-            orc.nonlinear = lambda fields: tuple(h.copy() for h in Hl[:3])
-            orc.substep()
+        o, os_, hp, sub = ysolve_reference(base, ps, ss, state, Hl, isub, c)
         v, phi, omy = inputs.fluctuations(c, device=dev, zchunk=64)
         ch.set_state(v, phi, omy, c["U"], c["W"])
         del v, phi, omy
@@ -203,13 +320,9 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
         ch.debug_set_substep_index(isub)
         ch.debug_run_stage(B.STAGE_YSOLVE)
         gv, gphi, gomy, gU, gW = ch.get_state()
-        e = {"v": rel(take_lines(gv, ps, ss), o.v), "phi": rel(take_lines(gphi, ps, ss), o.phi),
-             "omy": rel(take_lines(gomy, ps, ss), o.omy), "U": rel(gU, o.U)}
-        fl = {"v": rel(t.v, o.v), "phi": rel(t.phi, o.phi), "omy": rel(t.omy, o.omy), "U": rel(t.U, o.U)}
+        gpu = (take_lines(gv, ps, ss), take_lines(gphi, ps, ss), take_lines(gomy, ps, ss), gU.cpu().numpy())
         del gv, gphi, gomy
-        print(f"{name} substep {isub}: |gpu-oracle| {e}  |twin-oracle| {fl}")
-        for k in e:
-            assert e[k] < max(TOL_SUBSTEP, 2.0 * fl[k]), (isub, k, e, fl)
+        gate_ysolve(name, isub, gpu, o, os_, hp, sub)
         assert rel(take_lines(ch.debug_get_field(B.F_HV_PREV), ps, ss), o.hv_prev) < 1e-11
         assert rel(take_lines(ch.debug_get_field(B.F_HG_PREV), ps, ss), o.hg_prev) < 1e-13
         # the new state's derived fields (a1 chained behind the y-solve) on the same lines
@@ -223,7 +336,8 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
 def test_config5_whole_on_sampled_lines_and_planes(B):
     """The full 1536 x 1025 x 1152 config 5 in bench.py's launch configuration.  Memory-lean variant of the two tests
     above: the state is staged in host memory (chan_set_state_host), every other full-size field lives on the device
-    one at a time and is regenerated from its seed when it is needed again."""
+    one at a time and is regenerated from its seed when it is needed again.  4096 lines, all three substep
+    coefficient sets; 64 planes with the chunk seams."""
     env = os.environ.get("CHAN_TEST_FULLSIZE")
     if env and "cfg5" not in env.split(","):
         pytest.skip("CHAN_TEST_FULLSIZE excludes cfg5")
@@ -233,13 +347,13 @@ def test_config5_whole_on_sampled_lines_and_planes(B):
     shape = (nz, c["nx"] // 2, ny)
     if torch.cuda.mem_get_info(dev)[0] < 176e9:
         pytest.skip("config 5 needs its 148 GB workspace plus one 14.5 GB field and the filter output on the device")
-    hv, hp, ho = (torch.empty(shape, dtype=torch.complex128) for _ in range(3))
-    inputs.fluctuations(c, device=dev, zchunk=16, out=(hv, hp, ho))
+    hv, hp_, ho = (torch.empty(shape, dtype=torch.complex128) for _ in range(3))
+    inputs.fluctuations(c, device=dev, zchunk=16, out=(hv, hp_, ho))
     hU, hW = torch.from_numpy(c["U"]).clone(), torch.from_numpy(c["W"]).clone()
     torch.cuda.empty_cache()
     ch = B.Channel(c["nx"], ny, nz, c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
     ps, ss = sub_lattice(c)
-    sv, sphi, somy = (take_lines(t, ps, ss) for t in (hv, hp, ho))
+    state = tuple(take_lines(t, ps, ss) for t in (hv, hp_, ho))
     base = line_oracle(c, ps, ss)
 
     def gpu_lines(fid):
@@ -248,15 +362,15 @@ def test_config5_whole_on_sampled_lines_and_planes(B):
         del g
         return out
 
-    # ---- lines: a1-a2, then a9-a12 for the first and the last substep coefficient sets
-    ch.set_state_host(hv, hp, ho, hU, hW)
+    # ---- lines: a1-a2, then a9-a12 for the three substep coefficient sets
+    ch.set_state_host(hv, hp_, ho, hU, hW)
     o = copy.deepcopy(base)
-    o.set_state(sv, sphi, somy, c["U"], c["W"])
+    o.set_state(*state, c["U"], c["W"])
     for fid, ref in zip((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ), o.velocities_vorticities()):
         assert rel(gpu_lines(fid), ref) < 1e-12, fid
     fids = (B.F_H1, B.F_H2, B.F_H3, B.F_HV_PREV, B.F_HG_PREV)
-    for isub in (0, 2):
-        ch.set_state_host(hv, hp, ho, hU, hW)
+    for isub in (0, 1, 2):
+        ch.set_state_host(hv, hp_, ho, hU, hW)
         Hl = []
         for k, fid in enumerate(fids):
             f = random_field(shape, nz, 2000 + k, dev, scale=1e2 if k < 3 else 1.0)
@@ -266,27 +380,16 @@ def test_config5_whole_on_sampled_lines_and_planes(B):
             ch.debug_set_field(fid, f)
             del f
             torch.cuda.empty_cache()
-        o, t = copy.deepcopy(base), copy.deepcopy(base)
-        t.__class__ = TwinOracle
-        for orc in (o, t):
-            orc.set_state(sv, sphi, somy, c["U"], c["W"])
-            orc.isub = isub
-            orc.hv_prev, orc.hg_prev = Hl[3].copy(), Hl[4].copy()
-            orc.nonlinear = lambda fields: tuple(h.copy() for h in Hl[:3])
-            orc.substep()
+        o, os_, hp, sub = ysolve_reference(base, ps, ss, state, Hl, isub, c)
         ch.debug_set_substep_index(isub)
         ch.debug_run_stage(B.STAGE_YSOLVE)
-        e = {"v": rel(gpu_lines(B.F_V), o.v), "phi": rel(gpu_lines(B.F_PHI), o.phi), "omy": rel(gpu_lines(B.F_OMY), o.omy)}
+        gl = [gpu_lines(B.F_V), gpu_lines(B.F_PHI), gpu_lines(B.F_OMY)]
         ch.debug_run_stage(B.STAGE_DERIVE)
         ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
         prof, _ = ch.stats(B.STATS_READ)
-        e["U"] = rel(prof[0], o.U)                   # <u>(y) is the mean profile
-        fl = {"v": rel(t.v, o.v), "phi": rel(t.phi, o.phi), "omy": rel(t.omy, o.omy), "U": rel(t.U, o.U)}
-        print(f"cfg5 substep {isub}: |gpu-oracle| {e}  |twin-oracle| {fl}")
-        for k in e:
-            assert e[k] < max(TOL_SUBSTEP, 2.0 * fl[k]), (isub, k, e, fl)
+        gate_ysolve("cfg5", isub, (*gl, prof[0]), o, os_, hp, sub)        # <u>(y) is the mean profile
     # ---- planes: filter, statistics, nonlinear term from six seeded random fields
-    planes = sorted({0, 1, 2, ny // 3, ny // 2, 2 * ny // 3, ny - 3, ny - 2, ny - 1})
+    planes = sample_planes(ny, ch.debug_get_tuning()["planes_per_chunk"])
     sampled = []
     for k, fid in enumerate((B.F_U, B.F_V, B.F_W, B.F_OMX, B.F_OMY, B.F_OMZ)):
         f = random_field(shape, nz, 1000 + k, dev)
@@ -294,45 +397,39 @@ def test_config5_whole_on_sampled_lines_and_planes(B):
         sampled.append(f[:, :, planes].cpu().numpy())
         del f
         torch.cuda.empty_cache()
-    op = ChannelOracle(c["nx"], len(planes), nz, c["lx"], c["lz"], np.linspace(-1, 1, len(planes)), c["re"], c["dt"])
-    kxc, kzc = c["cut"]
-    got = ch.filter_store(kxc, kzc)
-    gp = got[:, planes].cpu().numpy()
-    del got
-    slots = [q % nz for q in list(range(0, kzc + 1)) + list(range(-kzc, 0))]
-    for n in range(3):
-        assert np.array_equal(gp[n], np.transpose(sampled[n][slots][:, : kxc + 1, :], (2, 0, 1))), n
-    pu, pv, pw, pox, poy, poz = (op.to_physical(f) for f in sampled)
-    for n, pr in enumerate((pu * pu, pu * pv, pu * pw, pv * pv, pv * pw, pw * pw, pox * pox + poy * poy + poz * poz)):
-        assert rel(gp[3 + n], op.to_spectral(pr, kxc, kzc)) < 1e-13, n
-    ch.debug_run_stage(B.STAGE_NONLINEAR)
-    for fid, ref_h in zip((B.F_H1, B.F_H2, B.F_H3), op.nonlinear(sampled)):
-        g = ch.debug_get_field(fid)
-        assert rel(g[:, :, planes], ref_h) < 1e-13, fid
-        del g
+    planes_check(B, ch, c, planes, sampled)
     ch.close()
 
 
-def test_fullsize_chained_substep_equals_the_staged_one(B):
-    """Property at full size (config 3): chan_substep hands D1-forward(v) from the last y sweep straight to the a1
-    sweeps; running the three stages one by one through the debug hooks recomputes it from the stored v.  Both must
-    give the same fields bit for bit (the stages themselves are checked against the oracle above)."""
-    c = inputs.config("cfg3")
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_fullsize_chained_substep_equals_the_staged_one(B, name):
+    """Property at full size: chan_substep hands D1-forward(v) from the last y sweep straight to the a1 sweeps; running
+    the three stages one by one through the debug hooks recomputes it from the stored v.  Both must give the same
+    fields bit for bit (the stages themselves are checked against the oracle above).  Config 4 has several plane chunks
+    with a ragged last one."""
+    c = inputs.config(name)
     dev = torch.device("cuda:0")
     v, phi, omy = inputs.fluctuations(c, device=dev, zchunk=64)
+    hv, hphi, homy = v.cpu(), phi.cpu(), omy.cpu()
+    del v, phi, omy
     res = []
+    fields = (B.F_V, B.F_PHI, B.F_OMY, B.F_U, B.F_W, B.F_OMX, B.F_OMZ)
     for chained in (True, False):
+        torch.cuda.empty_cache()
         ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"]).bind(dev)
-        ch.set_state(v, phi, omy, c["U"], c["W"])
-        ch._keep = None
+        ch.set_state_host(hv, hphi, homy, torch.from_numpy(c["U"]).clone(), torch.from_numpy(c["W"]).clone())
         if chained:
             ch.substep()
         else:
             ch.debug_run_stage(B.STAGE_NONLINEAR)
             ch.debug_run_stage(B.STAGE_YSOLVE)
             ch.debug_run_stage(B.STAGE_DERIVE)
-        res.append([ch.debug_get_field(f).cpu() for f in (B.F_V, B.F_PHI, B.F_OMY, B.F_U, B.F_W, B.F_OMX, B.F_OMZ)])
+        out = []
+        for f in fields:
+            g = ch.debug_get_field(f)
+            out.append(g.cpu())
+            del g
+        res.append(out)
         ch.close()
-        torch.cuda.empty_cache()
     for a, b in zip(*res):
         assert torch.equal(a, b)

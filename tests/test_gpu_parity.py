@@ -44,54 +44,69 @@ def seeded_state(c, boost=1.0):
     return v, phi, omy
 
 
-class TwinOracle(ChannelOracle):
-    """The same oracle with every banded solve done by LAPACK's dense pivoted LU instead of the unpivoted
-    band elimination: a second, equally legitimate fp64 evaluation order.  |oracle - twin| is the fp64
-    noise floor of the method on the given data: phi = lap(v) amplifies roundoff
-    in v by ||D2|| ~ 1/dy_min^2, and the O(U^2) mean-flow product leaks eps*U^2 into every small mode."""
-
-    def substep(self):
-        from oracle import compact_fd as cfd
-        orig = cfd.banded_solve
-
-        def dense(T, r):
-            T = np.asarray(T)
-            if T.ndim == 2:
-                shp = r.shape
-                return np.linalg.solve(cfd.band_to_dense(T), r.reshape(-1, shp[-1]).T).T.reshape(shp)
-            out = np.empty_like(r)
-            for b in range(T.shape[0]):
-                out[b] = np.linalg.solve(cfd.band_to_dense(T[b]), r[b].T).T
-            return out
-
-        cfd.banded_solve = dense
-        try:
-            super().substep()
-        finally:
-            cfd.banded_solve = orig
+# ---- fp64 rounding yardstick ------------------------------------------------------------------------------
+# phi^ = lap(v^) comes out of Helmholtz problems whose condition number grows like 1/dy_min^2 and of the 2x2
+# influence matrix, so BOTH fp64 evaluations (oracle and kernels) carry a rounding error on phi^ that can exceed
+# north_star's 1e-11 per substep (on config 1 the oracle itself is 4e-11 away from the exact discrete solution after
+# three substeps).  oracle.channel_hp.ChannelHP evaluates the same discrete steps in 80-bit long double (pinned
+# against exact rational arithmetic in tests/test_oracle_hp.py); |oracle - hp| is the oracle's own rounding error on
+# the given data.  Gate: |gpu - oracle| and |gpu - hp| <= max(1e-11 n, K_FLOOR |oracle - hp|).
+K_FLOOR = 4.0
+# the same per (kx,kz) line, so that low-energy modes are checked and not hidden in the whole-field norm
+K_LINE = 8.0
 
 
-def make_twin(c):
-    return TwinOracle(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+def make_hp(o):
+    from oracle.channel_hp import ChannelHP
+    return ChannelHP(o)
 
 
-def noise_floor(o, t):
-    return {"v": rel(t.v, o.v), "phi": rel(t.phi, o.phi), "omy": rel(t.omy, o.omy), "U": rel(t.U, o.U)}
+def noise_floor(o, h):
+    return {k: rel(getattr(o, k), np.asarray(getattr(h, k)).astype(np.asarray(getattr(o, k)).dtype)) for k in ("v", "phi", "omy", "U")}
 
 
-def check_state(ch, o, t, nsub, where):
-    """Gate: relative L2 <= 1e-11 per substep (north_star), or, where the method's own fp64 noise floor on
-    this data is above that, <= 2x the floor measured with the twin oracle."""
-    e = state_errors(ch, o)
-    f = noise_floor(o, t) if t is not None else {k: 0.0 for k in ("v", "phi", "omy", "U")}
-    for k in ("v", "phi", "omy", "U"):
-        assert e[k] < max(TOL_SUBSTEP * nsub, 2.0 * f[k]), (where, k, e, f)
+def line_rel(a, b):
+    """Relative L2 error of every (z slot, p) line: [nz][nxh]; lines where the reference vanishes count as 0."""
+    a = a.cpu().numpy() if isinstance(a, torch.Tensor) else np.asarray(a)
+    den = np.linalg.norm(b, axis=-1)
+    return np.linalg.norm(a - b, axis=-1) / np.where(den > 0, den, 1.0)
+
+
+def check_lines(gpu, o, h, nsub, where):
+    """Per-line gate: every line's |gpu - oracle| <= max(1e-11 n, K_LINE x that line's |oracle - hp|)."""
+    worst = {}
+    for k, g in zip(("v", "phi", "omy"), gpu):
+        ref = getattr(o, k)
+        e = line_rel(g, ref)
+        f = line_rel(np.asarray(getattr(h, k)).astype(complex), ref)
+        ratio = e / np.maximum(TOL_SUBSTEP * nsub, K_LINE * f)
+        worst[k] = float(ratio.max())
+        idx = np.unravel_index(np.argmax(ratio), ratio.shape)
+        assert worst[k] <= 1.0, (where, k, idx, float(e[idx]), float(f[idx]))
+    return worst
+
+
+def check_state(ch, o, h, nsub, where, lines=True):
+    """Gate: relative L2 <= 1e-11 per substep (north_star), or, where the oracle's own fp64 rounding error on this
+    data (|oracle - long-double evaluation|) is above that, <= K_FLOOR x that error; v and U are asserted against
+    the plain tolerance by the callers."""
+    gpu = ch.get_state()
+    e = state_errors(ch, o, gpu)
+    f = noise_floor(o, h) if h is not None else {k: 0.0 for k in ("v", "phi", "omy", "U")}
+    for k, g in zip(("v", "phi", "omy", "U"), gpu):
+        lim = max(TOL_SUBSTEP * nsub, K_FLOOR * f[k])
+        assert e[k] < lim, (where, k, e, f)
+        if h is not None:
+            assert rel(g, np.asarray(getattr(h, k)).astype(np.asarray(getattr(o, k)).dtype)) < lim, (where, k, "vs hp", e, f)
     assert e["W"] < 1e-12, (where, e)
+    if lines and h is not None:
+        e["worst_line_ratio"] = check_lines(gpu[:3], o, h, nsub, where)
+    print(f"{where}: |gpu-oracle| {e}  |oracle-hp| {f}")
     return e, f
 
 
-def state_errors(ch, o):
-    gv, gphi, gomy, gU, gW = ch.get_state()
+def state_errors(ch, o, gpu=None):
+    gv, gphi, gomy, gU, gW = gpu if gpu is not None else ch.get_state()
     return {"v": rel(gv, o.v), "phi": rel(gphi, o.phi), "omy": rel(gomy, o.omy), "U": rel(gU, o.U),
             "W": float(np.abs(gW.cpu().numpy() - o.W).max())}
 
@@ -194,7 +209,7 @@ def test_config1_ten_substeps_filter_and_stats(B):
     v, phi, omy = seeded_state(c)
     ch.set_state(v, phi, omy, c["U"], c["W"])
     o.set_state(v, phi, omy, c["U"], c["W"])
-    t = make_twin(c)
+    t = make_hp(o)
     t.set_state(v, phi, omy, c["U"], c["W"])
     for n in range(10):
         ch.substep()
@@ -234,7 +249,7 @@ def test_mid_full_steps_filter_stats(B):
     v, phi, omy = seeded_state(c)
     ch.set_state(v, phi, omy, c["U"], c["W"])
     o.set_state(v, phi, omy, c["U"], c["W"])
-    t = make_twin(c)
+    t = make_hp(o)
     t.set_state(v, phi, omy, c["U"], c["W"])
     for n in range(2):
         ch.step()
@@ -260,11 +275,17 @@ def test_ten_full_steps(B):
     v, phi, omy = seeded_state(c, 50.0)
     ch.set_state(v, phi, omy, c["U"], c["W"])
     o.set_state(v, phi, omy, c["U"], c["W"])
+    h = make_hp(o)
+    h.set_state(v, phi, omy, c["U"], c["W"])
     for _ in range(10):
         ch.step()
         o.step()
+        h.step()
     e = state_errors(ch, o)
     assert max(e["v"], e["phi"], e["omy"], e["U"]) < TOL_10STEPS, e
+    # per line as well (low-energy modes), against the oracle's own accumulated rounding error on each line
+    w = check_lines(ch.get_state()[:3], o, h, 30, "ten steps")
+    print("ten full steps: |gpu-oracle|", e, " |oracle-hp|", noise_floor(o, h), " worst line ratio", w)
     ch.close()
 
 
@@ -340,16 +361,19 @@ def test_host_buffer_entry_points(B):
     hv, hp, ho = (t.clone().pin_memory() for t in (v, phi, omy))
     hU, hW = torch.from_numpy(c["U"]).clone(), torch.from_numpy(c["W"]).clone()
     ch.set_state_host(hv, hp, ho, hU, hW)
+    # chan.h: the call synchronises, the host buffers are the caller's again at once -- scribble on them
+    for t in (hv, hp, ho, hU, hW):
+        t.fill_(7.0)
     o.set_state(v.numpy(), phi.numpy(), omy.numpy(), c["U"], c["W"])
     ch.step()
     o.step()
     ch.get_state_host(hv, hp, ho, hU, hW)
-    t = make_twin(c)
+    t = make_hp(o)
     t.set_state(v.numpy(), phi.numpy(), omy.numpy(), c["U"], c["W"])
     t.step()
     f = noise_floor(o, t)
-    assert rel(hv, o.v) < 3 * TOL_SUBSTEP and rel(ho, o.omy) < max(3 * TOL_SUBSTEP, 2 * f["omy"])
-    assert rel(hp, o.phi) < max(3 * TOL_SUBSTEP, 2 * f["phi"])
+    assert rel(hv, o.v) < 3 * TOL_SUBSTEP and rel(ho, o.omy) < max(3 * TOL_SUBSTEP, K_FLOOR * f["omy"])
+    assert rel(hp, o.phi) < max(3 * TOL_SUBSTEP, K_FLOOR * f["phi"])
     out = torch.empty((10, c["ny"], 2 * 8 + 1, 9), dtype=torch.complex128).pin_memory()
     ch.filter_store_host(8, 8, out)
     assert rel(out, o.filter_store(8, 8)) < 1e-10
@@ -365,7 +389,7 @@ def test_unlisted_transform_lengths_use_the_generic_kernels(B):
     v, phi, omy = seeded_state(c, 20.0)
     ch.set_state(v, phi, omy, c["U"], c["W"])
     o.set_state(v, phi, omy, c["U"], c["W"])
-    t = make_twin(c)
+    t = make_hp(o)
     t.set_state(v, phi, omy, c["U"], c["W"])
     ch.step()
     o.step()
@@ -424,12 +448,14 @@ def test_constant_pressure_gradient_forcing_and_narrow_stencils(B):
         if forcing:
             ch.set_pgrad(1.25)
             o.pgrad = 1.25
+        h = make_hp(o)                       # after pgrad: the yardstick copies the oracle's parameters
+        h.set_state(v, phi, omy, c["U"], c["W"])
         for _ in range(3):
             ch.substep()
             o.substep()
-        e = state_errors(ch, o)
+            h.substep()
+        e, f = check_state(ch, o, h, 3, (forcing, hl))
         assert max(e["v"], e["omy"], e["U"]) < 3 * TOL_SUBSTEP, (forcing, hl, e)
-        assert e["phi"] < 1e-9, (forcing, hl, e)
         assert ch.scalars()[0] == pytest.approx(o.pgrad, rel=1e-9)
         ch.close()
 

@@ -66,3 +66,26 @@ def test_band_tables_match_the_exact_rational_oracle_tables(lib, name):
         scale = np.maximum(np.abs(ref).max(axis=1, keepdims=True), 1e-300)  # A2/B2 wall rows are all zero
         assert (np.abs(got - ref) / scale).max() < 2e-15
     ch.close()
+
+
+def test_tuning_overrides_go_through_the_handle_not_the_environment(lib, monkeypatch):
+    """chan.h: "The library reads no environment variable and keeps no global state"."""
+    c = inputs.config("mid")
+    monkeypatch.setenv("CHAN_TZ", "1")            # the round-1 override: must be ignored now
+    monkeypatch.setenv("CHAN_CHUNK_MB", "1")
+    ch = binding.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    t0 = ch.debug_get_tuning()
+    assert t0["tz"] > 1 and t0["chunk_mb"] == 3072 and t0["planes_per_chunk"] == c["ny"] and t0["plane_streams"] == 1
+    need0 = ch.workspace_bytes()
+    ch.debug_set_tuning(tz=2, zthreads=128, chunk_mb=1, xfuse=4)
+    t1 = ch.debug_get_tuning()
+    assert (t1["tz"], t1["zthreads"], t1["chunk_mb"], t1["xfuse"]) == (2, 128, 1, 4)
+    assert 1 <= t1["planes_per_chunk"] < c["ny"] and ch.workspace_bytes() < need0
+    for bad in (dict(tz=3), dict(xfuse=5), dict(maxradix_z=13), dict(zthreads=16), dict(plane_streams=4)):
+        with pytest.raises(binding.ChanError) as e:
+            ch.debug_set_tuning(**bad)
+        assert e.value.status == binding.EINVAL
+        assert ch.debug_get_tuning() == t1        # a refused override leaves the handle unchanged
+    ch.debug_set_tuning()                         # all zeros: back to the plan's own choice
+    assert ch.debug_get_tuning() == t0 and ch.workspace_bytes() == need0
+    ch.close()
