@@ -135,7 +135,8 @@ typedef struct {
     int xthreads;         /* threads per CTA of the x pass, 32..256                                                */
     int chunk_mb;         /* size of the z-padded plane-chunk buffers in MiB (default 3072)                        */
     int planes_per_chunk; /* get only: y-planes per launch of the plane kernels that follows from chunk_mb         */
-    int plane_streams;    /* 1..3: internal streams the plane kernels of neighbouring chunks are spread over       */
+    int plane_overlap;    /* 1: K2, K3, K4 as separate launches; 2: merged launches (K2 of chunk t, K3 of chunk t-1, K4 of chunk
+                             t-2 interleaved in one grid; CHAN_EINVAL if not compiled for this plan); get: the mode in effect */
     int reserved[7];      /* must be 0                                                                             */
 } chan_tuning_t;
 int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t);
@@ -156,6 +157,8 @@ int chan_debug_run_stage(chan_t* h, int stage);
 int chan_debug_set_substep_index(chan_t* h, int i);
 /* Copy of the host-computed compact band tables, out[4][ny][7]: A1, B1, A2, B2 (HOST pointer). */
 int chan_debug_get_band_tables(const chan_t* h, double* host_out);
+/* One-line description of the plan in effect (stage lists, tiles, chunking) into buf[n] (HOST), NUL-terminated. */
+int chan_debug_describe(const chan_t* h, char* buf, size_t n);
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 long long chan_debug_launch_count(const chan_t* h);
 /* Per-kernel-class device timing with CUDA events on the bound stream (bench.py's roofline object).
@@ -164,7 +167,8 @@ long long chan_debug_launch_count(const chan_t* h);
  * milliseconds and the number of launches (arrays of CHAN_KC_COUNT entries, HOST pointers). */
 enum { CHAN_KC_D1FWD = 0, CHAN_KC_DERIVE_DOWN, CHAN_KC_DERIVE_UP, CHAN_KC_ZFFT_INV, CHAN_KC_XFFT_PROD, CHAN_KC_ZFFT_FWD,
        CHAN_KC_MEAN, CHAN_KC_Y1, CHAN_KC_Y2, CHAN_KC_Y3, CHAN_KC_Y4, CHAN_KC_Y5, CHAN_KC_TRANSPOSE,
-       CHAN_KC_FILTER_COPY, CHAN_KC_XFFT_PROD_FILTER, CHAN_KC_ZFFT_FWD_FILTER, CHAN_KC_STATS, CHAN_KC_COUNT };
+       CHAN_KC_FILTER_COPY, CHAN_KC_XFFT_PROD_FILTER, CHAN_KC_ZFFT_FWD_FILTER, CHAN_KC_STATS, CHAN_KC_PLANES_MERGED,
+       CHAN_KC_COUNT };
 int chan_debug_profile(chan_t* h, int enable);
 int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts);
 /* Plain line<->plane transposes (a2/a8) on caller buffers, for roofline timing: n fields of one

@@ -24,10 +24,10 @@ EXPORTS = [
     "chan_filter_store_host", "chan_step_filter", "chan_stats", "chan_get_scalars", "chan_set_pgrad", "chan_strerror",
     "chan_debug_get_field", "chan_debug_set_field", "chan_debug_run_stage", "chan_debug_set_substep_index",
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
-    "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning",
+    "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
-                  "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats"]
+                  "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged"]
 
 
 class Grid(C.Structure):
@@ -45,7 +45,7 @@ class Opts(C.Structure):
 class Tuning(C.Structure):
     """chan_tuning_t of include/chan.h (0 = the plan's own choice)."""
     _fields_ = [("xfuse", C.c_int), ("maxradix_z", C.c_int), ("maxradix_x", C.c_int), ("tz", C.c_int), ("zthreads", C.c_int),
-                ("xthreads", C.c_int), ("chunk_mb", C.c_int), ("planes_per_chunk", C.c_int), ("plane_streams", C.c_int),
+                ("xthreads", C.c_int), ("chunk_mb", C.c_int), ("planes_per_chunk", C.c_int), ("plane_overlap", C.c_int),
                 ("reserved", C.c_int * 7)]
 
 
@@ -95,6 +95,7 @@ def load():
         "chan_debug_profile_read": (i, [vp, vp, vp]),
         "chan_debug_set_tuning": (i, [vp, C.POINTER(Tuning)]),
         "chan_debug_get_tuning": (i, [vp, C.POINTER(Tuning)]),
+        "chan_debug_describe": (i, [vp, C.c_char_p, sz]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -139,6 +140,11 @@ class Channel:
         t = Tuning()
         _chk(self.lib.chan_debug_get_tuning(self.h, C.byref(t)), "chan_debug_get_tuning")
         return {k: getattr(t, k) for k, _ in Tuning._fields_ if k != "reserved"}
+
+    def debug_describe(self):
+        buf = C.create_string_buffer(512)
+        _chk(self.lib.chan_debug_describe(self.h, buf, 512), "chan_debug_describe")
+        return buf.value.decode()
 
     def workspace_bytes(self):
         return int(self.lib.chan_workspace_bytes(self.h))

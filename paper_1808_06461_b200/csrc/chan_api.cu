@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <string>
 #include <vector>
 
 #include "../../include/chan.h"
@@ -45,6 +46,8 @@ struct chan {
     void (*kzfwd)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int) = nullptr;
     void (*kx3)(PlaneParams, const double2*, int, double2*, int) = nullptr;
     void (*kx7)(PlaneParams, const double2*, int, double2*, int) = nullptr;
+    void (*kmerged)(PlaneParams, MergedArgs) = nullptr;   // K2 | K3 | K4 of neighbouring chunks in one launch, if compiled for this plan
+    bool merged = false;   // the substep's plane phase runs through kmerged
     bool zspecial = false, xspecial = false;
     chan_tuning_t tune = {};   // caller overrides (chan_debug_set_tuning), 0 = the plan's own choice
     // device pointers (carved)
@@ -83,7 +86,7 @@ void choose_tiling(chan_t* h) {
     h->Tz = U.tz ? U.tz : T;
     h->zthreads = U.zthreads ? U.zthreads : 256;
     h->xthreads = U.xthreads ? U.xthreads : (((size_t)3 * P.mx * 16 > 72 * 1024) ? 256 : 128);   // <= 3 CTAs per SM: use wider CTAs
-    const size_t per_plane = (size_t)13 * P.mz * P.nxh * 16;
+    const size_t per_plane = (size_t)(h->merged ? 19 : 13) * P.mz * P.nxh * 16;
     // zpad + xh: about 11 planes of config 5 per chunk (longer grids, smaller tails)
     const unsigned long long budget = (unsigned long long)(U.chunk_mb ? U.chunk_mb : 3072) << 20;
     long long pc = (long long)(budget / per_plane);
@@ -108,7 +111,8 @@ size_t carve(chan_t* h, char* base) {
     h->r1 = (double*)h->ox; h->r2 = h->r1 ? h->r1 + half : nullptr;
     h->r3 = (double*)h->w; h->r4 = h->r3 ? h->r3 + half : nullptr;
     h->coef = c.take<double4>((size_t)h->nm * 32);
-    h->zpad = c.take<double2>((size_t)6 * h->pc * P.mz * P.nxh * 16);
+    // merged plane launches double-buffer the chunks: two zpad sets; the two 3-field xh sets fit in the 7-field xh
+    h->zpad = c.take<double2>((size_t)(h->merged ? 12 : 6) * h->pc * P.mz * P.nxh * 16);
     h->xh = c.take<double2>((size_t)7 * h->pc * P.mz * P.nxh * 16);
     const size_t ny8 = (size_t)P.ny * 8;
     h->U = c.take<double>(ny8); h->W = c.take<double>(ny8); h->H1p = c.take<double>(ny8); h->H3p = c.take<double>(ny8);
@@ -191,6 +195,10 @@ int run_derive(chan_t* h) {
     X(4, 6, 8, 4) X(4, 6, 6, 8) X(4, 6, 8, 8) X(4, 12, 6, 6) X(4, 12, 6, 8) X(4, 12, 8, 8) X(8, 6, 1, 1) X(8, 12, 1, 1) X(8, 12, 6, 1) \
     X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 12, 16, 1) X(8, 16, 1, 1) X(8, 12, 8, 1) X(8, 6, 6, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
 
+// (z list | fused x radix, x list) pairs of config 5, 4, 3, of the "mid" parity case and of config 1
+#define CHAN_MERGED_PLANS(X) X(12, 12, 12, 1, 8, 6, 6, 8) X(6, 8, 8, 4, 8, 12, 16, 1) X(12, 12, 6, 1, 8, 12, 12, 1) X(12, 6, 1, 1, 4, 6, 6, 1) \
+    X(6, 8, 1, 1, 8, 6, 1, 1)
+
 typedef void (*zinv_fn)(PlaneParams, FieldPtrs, int, int, double2*, int);
 typedef void (*zfwd_fn)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int);
 typedef void (*xprod_fn)(PlaneParams, const double2*, int, double2*, int);
@@ -221,6 +229,21 @@ void pick_kernels(chan_t* h) {
         CHAN_XPLANS(X)
 #undef X
     }
+    // merged plane kernel: compiled for the (z list, x list) pairs of the benchmark shapes only (each pair is one more
+    // instantiation of all three bodies); any other plan runs the three kernels one after the other
+    h->kmerged = nullptr;
+    {
+        std::vector<int> head(P.fx.radix.begin(), P.fx.radix.end() - 1);
+#define X(z0, z1, z2, z3, f, x0, x1, x2) { const int rz[4] = {z0, z1, z2, z3}; const int rx[3] = {x0, x1, x2}; \
+        if (F == f && same_list(P.fz.radix, 4, rz) && same_list(head, 3, rx)) h->kmerged = k_planes_s<z0, z1, z2, z3, f, x0, x1, x2>; }
+        CHAN_MERGED_PLANS(X)
+#undef X
+    }
+}
+
+size_t merged_smem(const chan_t* h) {
+    const size_t a = (size_t)3 * h->P.mx * 16, b = (size_t)h->P.mz * h->Tz * 16;
+    return a > b ? a : b;
 }
 
 int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
@@ -290,10 +313,35 @@ int run_planes_both(chan_t* h, const FieldPtrsW& outH, const FieldPtrsW& outF, i
     return CHAN_OK;
 }
 
+// a3-a8 through the merged kernel: launch t carries K2 of chunk t, K3 of chunk t-1 and K4 of chunk t-2 (chan_fft.cuh);
+// chunk c uses zpad set c&1 and xh set c&1
+int run_planes_merged(chan_t* h, const FieldPtrsW& out) {
+    const Plan& P = h->P;
+    PlaneParams Q = pparams(h);
+    const int pc = h->pc, nch = (P.ny + pc - 1) / pc, T = h->Tz;
+    const size_t zset = (size_t)6 * pc * P.mz * P.nxh, xset = (size_t)3 * pc * P.mz * P.nxh;
+    auto planes_of = [&](int c) { return (P.ny - c * pc < pc) ? P.ny - c * pc : pc; };
+    const size_t sm = merged_smem(h);
+    for (int t = 0; t < nch + 2; ++t) {
+        MergedArgs A = {};
+        A.T = T; A.tiles = (unsigned)((P.nxh + T - 1) / T); A.scale = 1.0 / ((double)P.mx * (double)P.mz);
+        A.in.f[0] = h->u; A.in.f[1] = h->v; A.in.f[2] = h->w; A.in.f[3] = h->ox; A.in.f[4] = h->omy; A.in.f[5] = h->oz;
+        A.out = out;
+        if (t < nch) { A.j2 = t * pc; A.npl2 = planes_of(t); A.zw = h->zpad + (size_t)(t & 1) * zset; A.n2 = A.tiles * (unsigned)A.npl2 * 6u; }
+        if (t >= 1 && t <= nch) {
+            const int c = t - 1;
+            A.npl3 = planes_of(c); A.zr = h->zpad + (size_t)(c & 1) * zset; A.xw = h->xh + (size_t)(c & 1) * xset; A.n3 = (unsigned)P.mz * (unsigned)A.npl3;
+        }
+        if (t >= 2) { const int c = t - 2; A.j4 = c * pc; A.npl4 = planes_of(c); A.xr = h->xh + (size_t)(c & 1) * xset; A.n4 = A.tiles * (unsigned)A.npl4 * 3u; }
+        PB(CHAN_KC_PLANES_MERGED); h->kmerged<<<A.n2 + A.n3 + A.n4, 256, sm, h->stream>>>(Q, A); LAUNCHED();
+    }
+    return CHAN_OK;
+}
+
 int run_nonlinear(chan_t* h) {
     FieldPtrsW out;
     out.f[0] = h->H1; out.f[1] = h->H2; out.f[2] = h->H3;
-    return run_planes(h, 3, out, 0, 0);
+    return h->merged ? run_planes_merged(h, out) : run_planes(h, 3, out, 0, 0);
 }
 
 // a9-a12
@@ -338,8 +386,10 @@ double2* field_ptr(const chan_t* h, int f) {
 // tiling, kernel dispatch, size limits and workspace layout for the current plan and tuning overrides
 int configure(chan_t* h) {
     if ((int)h->P.fx.radix.size() > CHAN_MAX_STAGES || (int)h->P.fz.radix.size() > CHAN_MAX_STAGES) return CHAN_EINVAL;
-    choose_tiling(h);
     pick_kernels(h);
+    if (h->tune.plane_overlap == 2 && !h->kmerged) return CHAN_EINVAL;
+    h->merged = h->kmerged && h->tune.plane_overlap != 1;
+    choose_tiling(h);
     if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * h->Tz * 16 > 220 * 1024) return CHAN_EINVAL;
     if ((size_t)15 * h->P.ny * 8 > 220 * 1024) return CHAN_EINVAL;   // mean-mode solve lives in shared memory
     h->need = carve(h, nullptr);
@@ -390,7 +440,7 @@ int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t) {
     if ((t->xfuse && t->xfuse != 4 && t->xfuse != 8) || (t->maxradix_z && (t->maxradix_z < 2 || t->maxradix_z > 12)) ||
         (t->maxradix_x && (t->maxradix_x < 2 || t->maxradix_x > 16)) || (t->tz && !pow2(t->tz)) ||
         (t->zthreads && (t->zthreads < 32 || t->zthreads > 256)) || (t->xthreads && (t->xthreads < 32 || t->xthreads > 256)) ||
-        t->chunk_mb < 0 || t->plane_streams < 0 || t->plane_streams > 3)
+        t->chunk_mb < 0 || t->plane_overlap < 0 || t->plane_overlap > 2)
         return CHAN_EINVAL;
     const chan_tuning_t old = h->tune;
     const FftPlan ofx = h->P.fx, ofz = h->P.fz;
@@ -410,7 +460,7 @@ int chan_debug_get_tuning(const chan_t* h, chan_tuning_t* out) {
     out->tz = h->Tz; out->zthreads = h->zthreads; out->xthreads = h->xthreads;
     out->chunk_mb = h->tune.chunk_mb ? h->tune.chunk_mb : 3072;
     out->planes_per_chunk = h->pc;
-    out->plane_streams = h->tune.plane_streams ? h->tune.plane_streams : 1;
+    out->plane_overlap = h->merged ? 2 : 1;
     return CHAN_OK;
 }
 
@@ -448,6 +498,7 @@ int chan_bind(chan_t* h, void* dev_workspace, size_t bytes, void* cuda_stream) {
     CK(cudaFuncSetAttribute((const void*)h->kx3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)3 * P.mx * 16)));
     CK(cudaFuncSetAttribute((const void*)h->kx7, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)4 * P.mx * 16)));
     CK(cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)15 * P.ny * 8)));
+    if (h->merged) CK(cudaFuncSetAttribute((const void*)h->kmerged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)merged_smem(h)));
     h->bound = true; h->have_state = false; h->isub = 0; h->nsamples = 0;
     return CHAN_OK;
 }
@@ -676,6 +727,22 @@ int chan_debug_get_band_tables(const chan_t* h, double* out) {
 }
 
 long long chan_debug_launch_count(const chan_t* h) { return h ? h->launches : 0; }
+
+int chan_debug_describe(const chan_t* h, char* buf, size_t n) {
+    if (!h || !buf || n == 0) return CHAN_EINVAL;
+    std::string s = "x:";
+    const auto& rx = h->P.fx.radix; const auto& rz = h->P.fz.radix;
+    for (size_t k = 0; k + 1 < rx.size(); ++k) s += (k ? "," : " ") + std::to_string(rx[k]);
+    s += " |" + std::to_string(rx.back()) + "  z:";
+    for (size_t k = 0; k < rz.size(); ++k) s += (k ? "," : " ") + std::to_string(rz[k]);
+    s += "  specialised x/z: " + std::to_string((int)h->xspecial) + "/" + std::to_string((int)h->zspecial);
+    s += "  merged plane launches: " + std::to_string((int)h->merged);
+    s += "  tz " + std::to_string(h->Tz) + "  threads x/z " + std::to_string(h->xthreads) + "/" + std::to_string(h->zthreads);
+    s += "  planes per chunk " + std::to_string(h->pc);
+    std::strncpy(buf, s.c_str(), n - 1);
+    buf[n - 1] = 0;
+    return CHAN_OK;
+}
 
 int chan_debug_profile(chan_t* h, int enable) {
     if (!h) return CHAN_EINVAL;

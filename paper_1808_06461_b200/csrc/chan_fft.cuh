@@ -357,11 +357,13 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_g(CHAN_ZARGS_FWD) {
     }
 }
 
+// Bodies with explicit block coordinates (bx = column tile, jc = plane of the chunk, fi = field), shared by the
+// stand-alone kernels below and by the merged plane kernel k_planes_s.
 template <int R0, int R1, int R2, int R3>
-__global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
-    extern __shared__ double2 smem_raw[];
+__device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs& in, int j0, int npl, double2* __restrict__ zpad, int T,
+                                          double2* smem_raw, int bx, int jc, int fi) {
     constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
-    const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
+    const int p0 = bx * T;
     ZInvIO io = make_zinv_io(P, T, reinterpret_cast<c2*>(smem_raw), in.f[fi] + (size_t)(j0 + jc) * P.nm,
                              zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
@@ -385,10 +387,10 @@ __global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
     }
 }
 template <int R0, int R1, int R2, int R3>
-__global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
-    extern __shared__ double2 smem_raw[];
+__device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* __restrict__ xh, int pin, int j0, int npl, const FieldPtrsW& out,
+                                          double scale, int filt, int kxc, int kzc, int T, double2* smem_raw, int bx, int jc, int fi) {
     constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
-    const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
+    const int p0 = bx * T;
     const int j = j0 + jc;
     ZFwdIO io = make_zfwd_io(P, T, reinterpret_cast<c2*>(smem_raw), xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin,
                              filt ? out.f[fi] + (size_t)j * (2 * kzc + 1) * (kxc + 1) : out.f[fi] + (size_t)j * P.nm, pin, p0, scale,
@@ -413,6 +415,16 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
     }
     io.gout = true;
     zpass<R0, false, true, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
+}
+template <int R0, int R1, int R2, int R3>
+__global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
+    extern __shared__ double2 smem_raw[];
+    zinv_body<R0, R1, R2, R3>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+}
+template <int R0, int R1, int R2, int R3>
+__global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
+    extern __shared__ double2 smem_raw[];
+    zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, filt, kxc, kzc, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
 }
 #endif
 
@@ -580,10 +592,9 @@ __global__ void __launch_bounds__(256, 2) k_xfft_prod_g(CHAN_XARGS) {
 // stage radices as template parameters: R0, R1, R2 (1 = absent) then the fused radix F
 // (the filter variant keeps four sequences in shared memory: where only one such CTA fits on an SM it runs 512 threads)
 template <int NPROD, int F, int R0, int R1, int R2>
-__global__ void __launch_bounds__(NPROD == 7 ? 512 : 256, NPROD == 7 ? 1 : 2) k_xfft_prod_s(CHAN_XARGS) {
-    extern __shared__ double2 smem_raw[];
+__device__ __forceinline__ void xprod_body(const PlaneParams& P, const double2* __restrict__ zpad, int npl, double2* __restrict__ xh, int pout,
+                                           double2* smem_raw, int r, int jc) {
     constexpr int NC = (NPROD + 1) / 2;
-    const int r = blockIdx.x, jc = blockIdx.y;
     constexpr int M2 = F, M1 = R2 * F, M0 = R1 * R2 * F, mx = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
     XIO io; io.sm = reinterpret_cast<c2*>(smem_raw); io.stride = mx;
@@ -599,6 +610,57 @@ __global__ void __launch_bounds__(NPROD == 7 ? 512 : 256, NPROD == 7 ? 1 : 2) k_
     if constexpr (R1 > 1) { xpass<R1, false, true, M1>(io, P.fx.st[1], mx, NC, tid, nt); __syncthreads(); }
     if constexpr (R0 > 1) { io.zout = true; xpass<R0, false, true, M0>(io, P.fx.st[0], mx, NC, tid, nt); io.zout = false; __syncthreads(); }
     xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
+}
+template <int NPROD, int F, int R0, int R1, int R2>
+__global__ void __launch_bounds__(NPROD == 7 ? 512 : 256, NPROD == 7 ? 1 : 2) k_xfft_prod_s(CHAN_XARGS) {
+    extern __shared__ double2 smem_raw[];
+    xprod_body<NPROD, F, R0, R1, R2>(P, zpad, npl, xh, pout, smem_raw, blockIdx.x, blockIdx.y);
+}
+
+// =====================================================================================================
+// Merged plane kernel: one launch carries the inverse z pass (K2) of plane chunk t, the x pass with the products
+// (K3) of chunk t-1 and the forward z pass (K4) of chunk t-2, whose CTAs are INTERLEAVED in block-index order so
+// that every SM hosts a mix of them: K3 is bound by the shared-memory pipe (DRAM ~20% busy), K2 and K4 by memory
+// latency (shared-memory pipe half idle); running them side by side on an SM fills both units.  The three parts
+// work on different chunk buffers (zpad and xh are double-buffered by the host loop), so a launch has no internal
+// dependency; the order of launches on the stream carries the K2 -> K3 -> K4 dependency of each chunk.
+// Block b of the merged grid: A-blocks (K3) sit at the positions where floor(b n3/n) steps, the others are
+// B-blocks, first the n2 of K2, then the n4 of K4.
+// =====================================================================================================
+struct MergedArgs {
+    // K2: chunk starting at plane j2, npl2 planes, writes zw
+    FieldPtrs in; int j2, npl2; double2* zw;
+    // K3: reads zr, writes xw, npl3 planes
+    const double2* zr; int npl3; double2* xw;
+    // K4: reads xr, chunk starting at plane j4, npl4 planes
+    const double2* xr; int j4, npl4; FieldPtrsW out; double scale;
+    int T;
+    unsigned n2, n3, n4;      // blocks of each part (0: part absent from this launch)
+    unsigned tiles;           // column tiles per plane of the z passes
+};
+template <int Z0, int Z1, int Z2, int Z3, int F, int X0, int X1, int X2>
+__global__ void __launch_bounds__(256, 2) k_planes_s(PlaneParams P, MergedArgs A) {
+    extern __shared__ double2 smem_raw[];
+    const unsigned long long n = (unsigned long long)A.n2 + A.n3 + A.n4, b = blockIdx.x;
+    const unsigned a0 = (unsigned)(b * A.n3 / n), a1 = (unsigned)((b + 1) * A.n3 / n);
+    if (a1 > a0) {                                    // A-block number a0: row r of plane jc
+        const int jc = (int)(a0 / (unsigned)P.mz), r = (int)(a0 - (unsigned)jc * P.mz);
+        xprod_body<3, F, X0, X1, X2>(P, A.zr, A.npl3, A.xw, P.nxh, smem_raw, r, jc);
+        return;
+    }
+    unsigned ib = (unsigned)(b - a0);                 // B-block number
+    if (ib < A.n2) {
+        const unsigned per = A.tiles * (unsigned)A.npl2;
+        const int fi = (int)(ib / per); ib -= (unsigned)fi * per;
+        const int jc = (int)(ib / A.tiles), bx = (int)(ib - (unsigned)jc * A.tiles);
+        zinv_body<Z0, Z1, Z2, Z3>(P, A.in, A.j2, A.npl2, A.zw, A.T, smem_raw, bx, jc, fi);
+    } else {
+        ib -= A.n2;
+        const unsigned per = A.tiles * (unsigned)A.npl4;
+        const int fi = (int)(ib / per); ib -= (unsigned)fi * per;
+        const int jc = (int)(ib / A.tiles), bx = (int)(ib - (unsigned)jc * A.tiles);
+        zfwd_body<Z0, Z1, Z2, Z3>(P, A.xr, P.nxh, A.j4, A.npl4, A.out, A.scale, 0, 0, 0, A.T, smem_raw, bx, jc, fi);
+    }
 }
 #endif
 

@@ -73,12 +73,18 @@ def line_rel(a, b):
 
 
 def check_lines(gpu, o, h, nsub, where):
-    """Per-line gate: every line's |gpu - oracle| <= max(1e-11 n, K_LINE x that line's |oracle - hp|)."""
+    """Per-line gate: every line's relative error |gpu - oracle| <= max(1e-11 n, K_LINE x max(that line's |oracle - hp|,
+    the rms over all lines of |oracle - hp|)).  The realised rounding error of a single line scatters around the level
+    its conditioning sets (two independent fp64 evaluations of one line differ by up to ~10x in a few of 500 lines), so
+    the bound of a line is not allowed to fall below the field's typical level; a mode-local defect (a wrong
+    wavenumber, a dropped boundary row) is orders of magnitude above it."""
     worst = {}
     for k, g in zip(("v", "phi", "omy"), gpu):
         ref = getattr(o, k)
         e = line_rel(g, ref)
         f = line_rel(np.asarray(getattr(h, k)).astype(complex), ref)
+        live = np.linalg.norm(ref, axis=-1) > 0
+        f = np.maximum(f, np.sqrt(np.mean(f[live] ** 2)) if live.any() else 0.0)
         ratio = e / np.maximum(TOL_SUBSTEP * nsub, K_LINE * f)
         worst[k] = float(ratio.max())
         idx = np.unravel_index(np.argmax(ratio), ratio.shape)
@@ -483,4 +489,29 @@ def test_step_filter_is_filter_store_then_step_bit_for_bit(B, name):
             assert ex.value.status == B.ESTATE
         ch.close()
     for a, b in zip(*outs):
+        assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("name,chunk_mb", [("mid", 4), ("cfg1", 0)])
+def test_merged_plane_launches_equal_separate_launches_bit_for_bit(B, name, chunk_mb):
+    """chan_tuning_t.plane_overlap: launch t of the merged kernel carries the inverse z pass of plane chunk t, the x pass
+    of chunk t-1 and the forward z pass of chunk t-2 on double-buffered chunk buffers; the planes are independent, so
+    the result must not depend on the launch structure or on the chunk size ("mid" with 4 MiB chunks: 22 chunks of 3
+    planes with a ragged last one against 13 chunks of 5)."""
+    c = inputs.config(name)
+    v, phi, omy = seeded_state(c, 20.0 if name == "cfg1" else 1.0)
+    res = []
+    for overlap in (1, 2):
+        ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"],
+                       tuning=dict(plane_overlap=overlap, chunk_mb=chunk_mb)).bind("cuda:0")
+        t = ch.debug_get_tuning()
+        assert t["plane_overlap"] == overlap
+        if chunk_mb:
+            assert 1 < t["planes_per_chunk"] < c["ny"] and c["ny"] % t["planes_per_chunk"] != 0
+        ch.set_state(v, phi, omy, c["U"], c["W"])
+        ch.step()
+        db = ch.step_filter(*c["cut"])
+        res.append([db.clone()] + [x.clone() for x in ch.get_state()] + [ch.debug_get_field(f) for f in (B.F_H1, B.F_H2, B.F_H3)])
+        ch.close()
+    for a, b in zip(*res):
         assert torch.equal(a, b)

@@ -75,13 +75,13 @@ def test_tuning_overrides_go_through_the_handle_not_the_environment(lib, monkeyp
     monkeypatch.setenv("CHAN_CHUNK_MB", "1")
     ch = binding.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
     t0 = ch.debug_get_tuning()
-    assert t0["tz"] > 1 and t0["chunk_mb"] == 3072 and t0["planes_per_chunk"] == c["ny"] and t0["plane_streams"] == 1
+    assert t0["tz"] > 1 and t0["chunk_mb"] == 3072 and t0["planes_per_chunk"] == c["ny"] and t0["plane_overlap"] in (1, 2)
     need0 = ch.workspace_bytes()
     ch.debug_set_tuning(tz=2, zthreads=128, chunk_mb=1, xfuse=4)
     t1 = ch.debug_get_tuning()
     assert (t1["tz"], t1["zthreads"], t1["chunk_mb"], t1["xfuse"]) == (2, 128, 1, 4)
     assert 1 <= t1["planes_per_chunk"] < c["ny"] and ch.workspace_bytes() < need0
-    for bad in (dict(tz=3), dict(xfuse=5), dict(maxradix_z=13), dict(zthreads=16), dict(plane_streams=4)):
+    for bad in (dict(tz=3), dict(xfuse=5), dict(maxradix_z=13), dict(zthreads=16), dict(plane_overlap=3)):
         with pytest.raises(binding.ChanError) as e:
             ch.debug_set_tuning(**bad)
         assert e.value.status == binding.EINVAL
