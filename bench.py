@@ -37,12 +37,14 @@ UNIT = "Mpoint*substeps/s"
 BYTES_PER_POINT = {
     "d1_forward": 16, "derive_down": 48, "derive_up": 40, "zfft_inv": 120, "xfft_prod": 108, "zfft_fwd": 60,
     "y1": 56, "y2": 80, "y3": 88, "y4": 72, "stats": 48, "transpose": 16,   # y1..y4 = sweeps SA..SD, derive_* = SE, SF
+    "planes_merged": 288,     # K2 + K3 + K4 of neighbouring chunks in one launch (120 + 108 + 60)
 }
 SURVEY_GROUPS = {
     "K2 z-pad + inverse z-FFT": (["zfft_inv"], 120),
     "K3 x-FFT . products . x-FFT": (["xfft_prod"], 108),
     "K4 forward z-FFT + truncate": (["zfft_fwd"], 60),
     "K5+K1 y-phase": (["y1", "y2", "y3", "y4", "y5", "d1_forward", "derive_down", "derive_up", "mean"], 144),
+    "K2+K3+K4 plane phase": (["zfft_inv", "xfft_prod", "zfft_fwd", "planes_merged"], 288),
 }
 
 
@@ -242,6 +244,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft-line", action="store_true")
+    ap.add_argument("--tuning", default="", help="chan_tuning_t overrides, e.g. plane_overlap=1,maxradix_x=16 (experiments)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -285,7 +288,10 @@ def main():
     hU = torch.from_numpy(c["U"]).clone()
     hW = torch.from_numpy(c["W"]).clone()
     torch.cuda.empty_cache()
-    ch = binding.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"])
+    tuning = {k: int(v_) for k, v_ in (kv.split("=") for kv in args.tuning.split(",") if kv)}
+    ch = binding.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"], tuning=tuning or None)
+    plan_text, tune = ch.debug_describe(), ch.debug_get_tuning()
+    merged = tune["plane_overlap"] == 2
     ws_bytes = ch.workspace_bytes()
     ch.bind(dev)
     ch.set_state_host(hv, hp, ho, hU, hW)
@@ -343,15 +349,11 @@ def main():
     dom = max((k for k in sub_classes if k in BYTES_PER_POINT), key=lambda k: sub_classes[k][0])
     dms, dcnt = sub_classes[dom]
     launches_per_field = dcnt / K          # per step
-    # points one launch processes: y-phase kernels and stats see the whole field; plane kernels one chunk
-    if dom in ("zfft_inv",):
-        pts_per_launch = npts * 3 / launches_per_field      # 3 sweeps per step: the fused filter shares the first one
-    elif dom in ("xfft_prod", "zfft_fwd"):
-        pts_per_launch = npts * 3 / launches_per_field
-    elif dom == "stats":
-        pts_per_launch = npts
-    else:
-        pts_per_launch = npts
+    # points one launch processes: y-phase kernels and stats see the whole field; plane kernels one chunk.  With merged
+    # plane launches the first substep of chan_step_filter (which shares its z-padded planes with the filter) runs the
+    # separate kernels and the other two substeps the merged one.
+    plane_sweeps = {"zfft_inv": 1 if merged else 3, "xfft_prod": 1 if merged else 3, "zfft_fwd": 1 if merged else 3, "planes_merged": 2}
+    pts_per_launch = npts * plane_sweeps[dom] / launches_per_field if dom in plane_sweeps else npts
     abytes = BYTES_PER_POINT[dom] * pts_per_launch
     achieved = abytes / (dms / dcnt * 1e-3) / 1e9
     planes_per_launch = round(pts_per_launch / (c["nx"] * c["nz"]))
@@ -367,10 +369,14 @@ def main():
                             "flops_per_launch": fl, "peak_source": "derived: 148 SM x 64 FMA/clk x 2 x 1.965 GHz"}
     groups = {}
     for gname, (classes, bpp) in SURVEY_GROUPS.items():
+        if merged and gname.startswith(("K2 ", "K3 ", "K4 ")):
+            continue                                         # only one of three substeps runs them separately: see the plane-phase group
         gms = sum(prof[k][0] for k in classes if k in prof)
         if gms > 0:
             gb = bpp * npts * 3 * K / (gms * 1e-3) / 1e9     # substep part only: the filter has its own classes
             groups[gname] = {"ms_per_substep": gms / (3 * K), "survey_bytes_per_point": bpp, "achieved_GBs": gb, "frac": gb / peak}
+    sub_gb = 432 * npts / (ms_sub / (3 * K) * 1e-3) / 1e9    # 54 field passes = 432 B/point per substep
+    groups["substep total"] = {"ms_per_substep": ms_sub / (3 * K), "survey_bytes_per_point": 432, "achieved_GBs": sub_gb, "frac": sub_gb / peak}
     kernel_ms = {k: {"ms_per_step": v_[0] / K, "launches_per_step": v_[1] / K} for k, v_ in sub_classes.items()}
 
     # ---- end to end through the host-buffer entry points ---------------------------------------------
@@ -438,7 +444,8 @@ def main():
         "config": {"workload": wl, "grid": [c["nx"], c["ny"], c["nz"]], "padded": [3 * c["nx"] // 2, c["ny"], 3 * c["nz"] // 2],
                    "step": "chan_stats(ACCUMULATE) + chan_step_filter (= chan_filter_store of the entry state + 1 RK3 step of 3 substeps); value counts the 3 substeps",
                    "filter_cut": [kxc, kzc], "l2": "inputs larger than L2 (one field = %.2f GB)" % (F / 1e9),
-                   "workspace_GB": ws_bytes / 1e9, "multi_gpu": "replicas only", "state_finite": finite},
+                   "workspace_GB": ws_bytes / 1e9, "multi_gpu": "replicas only", "state_finite": finite, "plan": plan_text,
+                   "tuning": tune},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches),
         "substep_only": substep_only, "roofline": roofline, "roofline_groups": groups, "kernel_ms": kernel_ms,
         "cpu_baseline": cpu, "cufft_reference_line": cufft,

@@ -104,6 +104,28 @@ int chan_step_filter(chan_t* h, int kx_cut, int kz_cut, void* dev_out, size_t ou
  * CHAN_ENOSPACE if it is larger than max(one field, min(ten fields, 64 MiB)) -- use chan_filter_store then. */
 int chan_filter_store_host(chan_t* h, int kx_cut, int kz_cut, void* host_out, size_t out_bytes);
 
+/* Storage precision of the filtered database (NEXT-1; the paper's database holds about four bytes per
+ * value): bytes_per_real = 8 (default: complex128 output, as documented above) or 4: chan_filter_store,
+ * chan_step_filter, chan_filter_store_host and chan_run then write complex64 [10][ny][2 kz_cut+1][kx_cut+1] -- every
+ * value computed in fp64 exactly as before and rounded once, to nearest even, when it is stored; the mode selection
+ * is unchanged.  out_bytes / slot_bytes are checked against the smaller size.  CHAN_EINVAL for any other value. */
+int chan_set_filter_precision(chan_t* h, int bytes_per_real);
+
+/* Snapshot cadence (NEXT-1; filtered fields are stored every Delta t_e, a multiple of the time
+ * step; L47: statistics on the fly).  Runs nsteps full steps without a host round trip: before step n the
+ * statistics of the current state are accumulated if stats_every > 0 and n % stats_every == 0, and the filtered
+ * database of the current state is emitted (fused into the step, as chan_step_filter) into slot
+ * (emitted so far) % ring_slots of dev_ring if filter_every > 0 and n % filter_every == 0.  A slot is slot_bytes
+ * long and must hold one database in the precision in effect (CHAN_ENOSPACE otherwise); the caller drains the ring
+ * (e.g. by copies on another stream ordered by events) before it wraps.  *snapshots = databases emitted (may be
+ * NULL).  Everything is enqueued on the bound stream; nothing synchronises.  CHAN_ESTATE mid-step. */
+typedef struct {
+    int nsteps, filter_every, stats_every;
+    int kx_cut, kz_cut;
+    void* dev_ring; size_t slot_bytes; int ring_slots;
+} chan_run_t;
+int chan_run(chan_t* h, const chan_run_t* r, long long* snapshots);
+
 /* Plane statistics (a14; "Regular statistics of the fully resolved flow are computed and stored
  * on-the-fly"; the profiles are those of the ten variables of L124): flags is an OR of the values below.  ACCUMULATE adds the ten profiles
  * <u>,<v>,<w>,<uu>,<uv>,<uw>,<vv>,<vw>,<ww>,<om_i om_i> of the current state to the running sums;
@@ -129,14 +151,15 @@ const char* chan_strerror(int status);
 typedef struct {
     int xfuse;            /* 4 | 8: radix of the x stage fused with the products                                  */
     int maxradix_z;       /* 2..12: largest radix of a z stage                                                    */
-    int maxradix_x;       /* 2..16: largest radix of an x stage in front of the fused one                          */
+    int maxradix_x;       /* 2..18: largest radix of an x stage in front of the fused one                          */
     int tz;               /* k_x columns per z tile: 1, 2, 4, 8 or 16                                              */
     int zthreads;         /* threads per CTA of the z passes, 32..256                                              */
     int xthreads;         /* threads per CTA of the x pass, 32..256                                                */
     int chunk_mb;         /* size of the z-padded plane-chunk buffers in MiB (default 3072)                        */
     int planes_per_chunk; /* get only: y-planes per launch of the plane kernels that follows from chunk_mb         */
-    int plane_overlap;    /* 1: K2, K3, K4 as separate launches; 2: merged launches (K2 of chunk t, K3 of chunk t-1, K4 of chunk
-                             t-2 interleaved in one grid; CHAN_EINVAL if not compiled for this plan); get: the mode in effect */
+    int plane_overlap;    /* 1 (default): K2, K3, K4 as separate launches; 2: merged launches (K2 of chunk t, K3 of chunk t-1,
+                             K4 of chunk t-2 interleaved in one grid; CHAN_EINVAL if not compiled for this plan; results equal
+                             to rounding, not bit for bit: another kernel, another FMA contraction); get: the mode in effect */
     int reserved[7];      /* must be 0                                                                             */
 } chan_tuning_t;
 int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t);
@@ -171,6 +194,10 @@ enum { CHAN_KC_D1FWD = 0, CHAN_KC_DERIVE_DOWN, CHAN_KC_DERIVE_UP, CHAN_KC_ZFFT_I
        CHAN_KC_COUNT };
 int chan_debug_profile(chan_t* h, int enable);
 int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts);
+/* fp64 FMA throughput of the device, measured with a register-only micro-kernel (8 independent DFMA chains per thread,
+ * 8 CTAs of 256 threads per SM, about 30 ms, best of 3 after a warm-up round) on the bound stream; synchronises.
+ * TFLOP/s into *host_tflops.  The "alu" roof of bench.py. */
+int chan_debug_fma_peak(chan_t* h, double* host_tflops);
 /* Plain line<->plane transposes (a2/a8) on caller buffers, for roofline timing: n fields of one
  * [nz][nx/2][ny] <-> [ny][nz][nx/2] complex128 array each. dir 0: line->plane, 1: plane->line. */
 int chan_debug_transpose(chan_t* h, int dir, const void* dev_in, void* dev_out);

@@ -264,11 +264,14 @@ class ChannelOracle:
             self.substep()
 
     # ------------------------------------------------------------------ filter and statistics
-    def filter_store(self, kx_cut, kz_cut):
+    def filter_store(self, kx_cut, kz_cut, single=False):
         """ten variables, sharp cutoff 0<=p<=kx_cut, |q|<=kz_cut (readings R11, R12).
 
         Returns ``[10][ny][2 kz_cut + 1][kx_cut + 1]`` complex: u,v,w, uu,uv,uw,vv,vw,ww, om_i om_i.
         Products are formed on the dealiased grid at full resolution and truncated afterwards.
+        ``single``: the database as the paper stores it -- about four bytes per value (150 TB for
+        3900 snapshots of ten 1024^3-point variables; reading R13) -- i.e. the fp64 result rounded ONCE, to nearest
+        even, to IEEE binary32 per component (complex64).
         """
         assert 0 <= kx_cut <= self.nx // 2 - 1 and 0 <= kz_cut <= self.nz // 2 - 1
         u, v, w, ox, oy, oz = self.velocities_vorticities()
@@ -280,7 +283,21 @@ class ChannelOracle:
         prods = (pu * pu, pu * pv, pu * pw, pv * pv, pv * pw, pw * pw, pox * pox + poy * poy + poz * poz)
         for n, pr in enumerate(prods):
             out[3 + n] = self.to_spectral(pr, kx_cut, kz_cut)
-        return out
+        return out.astype(np.complex64) if single else out
+
+    def run(self, nsteps, filter_every, stats_every, kx_cut, kz_cut, single=False):
+        """Snapshot cadence (the filtered fields are stored every Delta t_e, a multiple of the time
+        step; L47: statistics on the fly): ``nsteps`` full steps; before step n the filtered database of the current
+        state is emitted when n % filter_every == 0 and the statistics are accumulated when n % stats_every == 0
+        (0 = never).  Returns the list of emitted databases."""
+        snaps = []
+        for n in range(nsteps):
+            if stats_every and n % stats_every == 0:
+                self.stats_accumulate()
+            if filter_every and n % filter_every == 0:
+                snaps.append(self.filter_store(kx_cut, kz_cut, single))
+            self.step()
+        return snaps
 
     def stats_profiles(self):
         """<u_i>, <u_i u_j>, <om_i om_i> per y-plane by Parseval sums over the retained modes."""

@@ -24,7 +24,7 @@ EXPORTS = [
     "chan_filter_store_host", "chan_step_filter", "chan_stats", "chan_get_scalars", "chan_set_pgrad", "chan_strerror",
     "chan_debug_get_field", "chan_debug_set_field", "chan_debug_run_stage", "chan_debug_set_substep_index",
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
-    "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe",
+    "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe", "chan_debug_fma_peak", "chan_set_filter_precision", "chan_run",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
                   "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged"]
@@ -47,6 +47,12 @@ class Tuning(C.Structure):
     _fields_ = [("xfuse", C.c_int), ("maxradix_z", C.c_int), ("maxradix_x", C.c_int), ("tz", C.c_int), ("zthreads", C.c_int),
                 ("xthreads", C.c_int), ("chunk_mb", C.c_int), ("planes_per_chunk", C.c_int), ("plane_overlap", C.c_int),
                 ("reserved", C.c_int * 7)]
+
+
+class Run(C.Structure):
+    """chan_run_t of include/chan.h."""
+    _fields_ = [("nsteps", C.c_int), ("filter_every", C.c_int), ("stats_every", C.c_int), ("kx_cut", C.c_int), ("kz_cut", C.c_int),
+                ("dev_ring", C.c_void_p), ("slot_bytes", C.c_size_t), ("ring_slots", C.c_int)]
 
 
 class ChanError(RuntimeError):
@@ -96,6 +102,9 @@ def load():
         "chan_debug_set_tuning": (i, [vp, C.POINTER(Tuning)]),
         "chan_debug_get_tuning": (i, [vp, C.POINTER(Tuning)]),
         "chan_debug_describe": (i, [vp, C.c_char_p, sz]),
+        "chan_debug_fma_peak": (i, [vp, C.POINTER(C.c_double)]),
+        "chan_set_filter_precision": (i, [vp, i]),
+        "chan_run": (i, [vp, C.POINTER(Run), C.POINTER(C.c_longlong)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -196,24 +205,47 @@ class Channel:
         _chk(self.lib.chan_step(self.h), "chan_step")
 
     # ---- filter and statistics ---------------------------------------------------------------------
-    def filter_store(self, kx_cut, kz_cut, out=None):
-        shape = (10, self.ny, 2 * kz_cut + 1, kx_cut + 1)
+    def set_filter_precision(self, bytes_per_real):
+        """8: complex128 database (default); 4: complex64 (rounded once from the fp64 result)."""
+        _chk(self.lib.chan_set_filter_precision(self.h, int(bytes_per_real)), "chan_set_filter_precision")
+        self._fdtype = torch.complex64 if bytes_per_real == 4 else torch.complex128
+
+    def _fout(self, kx_cut, kz_cut, out, lead=()):
+        dt = getattr(self, "_fdtype", torch.complex128)
         if out is None:
-            out = torch.empty(shape, dtype=torch.complex128, device=self.device)
-        _chk(self.lib.chan_filter_store(self.h, kx_cut, kz_cut, out.data_ptr(), out.numel() * 16), "chan_filter_store")
+            out = torch.empty(tuple(lead) + (10, self.ny, 2 * kz_cut + 1, kx_cut + 1), dtype=dt, device=self.device)
+        assert out.dtype == dt and out.is_contiguous()
+        return out
+
+    def filter_store(self, kx_cut, kz_cut, out=None):
+        out = self._fout(kx_cut, kz_cut, out)
+        _chk(self.lib.chan_filter_store(self.h, kx_cut, kz_cut, out.data_ptr(), out.numel() * out.element_size()), "chan_filter_store")
         return out
 
     def step_filter(self, kx_cut, kz_cut, out=None):
         """filter_store of the current state fused into the step that follows."""
-        shape = (10, self.ny, 2 * kz_cut + 1, kx_cut + 1)
-        if out is None:
-            out = torch.empty(shape, dtype=torch.complex128, device=self.device)
-        _chk(self.lib.chan_step_filter(self.h, kx_cut, kz_cut, out.data_ptr(), out.numel() * 16), "chan_step_filter")
+        out = self._fout(kx_cut, kz_cut, out)
+        _chk(self.lib.chan_step_filter(self.h, kx_cut, kz_cut, out.data_ptr(), out.numel() * out.element_size()), "chan_step_filter")
         return out
 
     def filter_store_host(self, kx_cut, kz_cut, out):
-        _chk(self.lib.chan_filter_store_host(self.h, kx_cut, kz_cut, _host_ptr(out), out.numel() * 16), "chan_filter_store_host")
+        _chk(self.lib.chan_filter_store_host(self.h, kx_cut, kz_cut, _host_ptr(out), out.numel() * out.element_size()),
+             "chan_filter_store_host")
         return out
+
+    def run(self, nsteps, filter_every, stats_every, kx_cut, kz_cut, ring=None, ring_slots=None):
+        """chan_run: nsteps full steps with the snapshot cadence; returns (ring tensor [slots][10][ny][..][..], emitted)."""
+        if filter_every > 0:
+            if ring is None:
+                slots = ring_slots or (nsteps + filter_every - 1) // filter_every
+                ring = self._fout(kx_cut, kz_cut, None, lead=(max(slots, 1),))
+            slots = ring.shape[0]
+            r = Run(nsteps, filter_every, stats_every, kx_cut, kz_cut, ring.data_ptr(), ring[0].numel() * ring.element_size(), slots)
+        else:
+            r = Run(nsteps, 0, stats_every, kx_cut, kz_cut, None, 0, 0)
+        n = C.c_longlong(0)
+        _chk(self.lib.chan_run(self.h, C.byref(r), C.byref(n)), "chan_run")
+        return ring, int(n.value)
 
     def stats(self, flags):
         out = np.zeros((10, self.ny))
@@ -251,6 +283,12 @@ class Channel:
         out = np.zeros((4, self.ny, 7))
         _chk(self.lib.chan_debug_get_band_tables(self.h, out.ctypes.data), "chan_debug_get_band_tables")
         return out
+
+    def debug_fma_peak(self):
+        """Measured fp64 FMA throughput of the device in TFLOP/s (register-only micro-kernel)."""
+        out = C.c_double(0.0)
+        _chk(self.lib.chan_debug_fma_peak(self.h, C.byref(out)), "chan_debug_fma_peak")
+        return float(out.value)
 
     def debug_launch_count(self):
         return int(self.lib.chan_debug_launch_count(self.h))

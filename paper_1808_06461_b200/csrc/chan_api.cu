@@ -49,6 +49,7 @@ struct chan {
     void (*kmerged)(PlaneParams, MergedArgs) = nullptr;   // K2 | K3 | K4 of neighbouring chunks in one launch, if compiled for this plan
     bool merged = false;   // the substep's plane phase runs through kmerged
     bool zspecial = false, xspecial = false;
+    int out_f32 = 0;           // filtered database as complex64 (chan_set_filter_precision)
     chan_tuning_t tune = {};   // caller overrides (chan_debug_set_tuning), 0 = the plan's own choice
     // device pointers (carved)
     double2 *v, *phi, *omy, *hv, *hg, *u, *w, *ox, *oz;   // plane layout fields
@@ -193,10 +194,10 @@ int run_derive(chan_t* h) {
     X(6, 8, 8, 4) X(6, 6, 8, 8) X(6, 8, 8, 8)
 #define CHAN_XPLANS(X) X(4, 6, 1, 1) X(4, 12, 1, 1) X(4, 6, 4, 1) X(4, 6, 6, 1) X(4, 6, 8, 1) X(4, 12, 8, 1) X(4, 6, 6, 4) X(4, 6, 6, 6) \
     X(4, 6, 8, 4) X(4, 6, 6, 8) X(4, 6, 8, 8) X(4, 12, 6, 6) X(4, 12, 6, 8) X(4, 12, 8, 8) X(8, 6, 1, 1) X(8, 12, 1, 1) X(8, 12, 6, 1) \
-    X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 12, 16, 1) X(8, 16, 1, 1) X(8, 12, 8, 1) X(8, 6, 6, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
+    X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 12, 16, 1) X(8, 18, 16, 1) X(8, 18, 1, 1) X(8, 16, 1, 1) X(8, 12, 8, 1) X(8, 6, 6, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
 
 // (z list | fused x radix, x list) pairs of config 5, 4, 3, of the "mid" parity case and of config 1
-#define CHAN_MERGED_PLANS(X) X(12, 12, 12, 1, 8, 6, 6, 8) X(6, 8, 8, 4, 8, 12, 16, 1) X(12, 12, 6, 1, 8, 12, 12, 1) X(12, 6, 1, 1, 4, 6, 6, 1) \
+#define CHAN_MERGED_PLANS(X) X(12, 12, 12, 1, 8, 6, 6, 8) X(12, 12, 12, 1, 8, 18, 16, 1) X(6, 8, 8, 4, 8, 12, 16, 1) X(12, 12, 6, 1, 8, 12, 12, 1) X(12, 6, 1, 1, 8, 18, 1, 1) \
     X(6, 8, 1, 1, 8, 6, 1, 1)
 
 typedef void (*zinv_fn)(PlaneParams, FieldPtrs, int, int, double2*, int);
@@ -286,7 +287,7 @@ int run_planes(chan_t* h, int nprod, const FieldPtrsW& out, int kxc, int kzc) {
         int rc = zinv(h, Q, in, 6, j0, npl);
         if (rc) return rc;
         if ((rc = xprod(h, Q, nprod, npl, pout))) return rc;
-        rc = zfwd(h, Q, pout, nprod, j0, npl, out, scale, nprod == 7, kxc, kzc);
+        rc = zfwd(h, Q, pout, nprod, j0, npl, out, scale, nprod == 7 ? 1 + h->out_f32 : 0, kxc, kzc);
         if (rc) return rc;
     }
     return CHAN_OK;
@@ -306,7 +307,7 @@ int run_planes_both(chan_t* h, const FieldPtrsW& outH, const FieldPtrsW& outF, i
         if (rc) return rc;
         // the filter products first: its z pass reads the small xh, then the H pass overwrites xh and (later) u, w, om_x
         if ((rc = xprod(h, Q, 7, npl, kxc + 1))) return rc;
-        if ((rc = zfwd(h, Q, kxc + 1, 7, j0, npl, outF, scale, 1, kxc, kzc))) return rc;
+        if ((rc = zfwd(h, Q, kxc + 1, 7, j0, npl, outF, scale, 1 + h->out_f32, kxc, kzc))) return rc;
         if ((rc = xprod(h, Q, 3, npl, P.nxh))) return rc;
         if ((rc = zfwd(h, Q, P.nxh, 3, j0, npl, outH, scale, 0, 0, 0))) return rc;
     }
@@ -388,7 +389,7 @@ int configure(chan_t* h) {
     if ((int)h->P.fx.radix.size() > CHAN_MAX_STAGES || (int)h->P.fz.radix.size() > CHAN_MAX_STAGES) return CHAN_EINVAL;
     pick_kernels(h);
     if (h->tune.plane_overlap == 2 && !h->kmerged) return CHAN_EINVAL;
-    h->merged = h->kmerged && h->tune.plane_overlap != 1;
+    h->merged = h->kmerged && h->tune.plane_overlap == 2;   // measured on config 5: no gain over separate launches, so opt-in
     choose_tiling(h);
     if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * h->Tz * 16 > 220 * 1024) return CHAN_EINVAL;
     if ((size_t)15 * h->P.ny * 8 > 220 * 1024) return CHAN_EINVAL;   // mean-mode solve lives in shared memory
@@ -438,7 +439,7 @@ int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t) {
     for (int r : t->reserved) if (r) return CHAN_EINVAL;
     auto pow2 = [](int v) { return v == 1 || v == 2 || v == 4 || v == 8 || v == 16; };
     if ((t->xfuse && t->xfuse != 4 && t->xfuse != 8) || (t->maxradix_z && (t->maxradix_z < 2 || t->maxradix_z > 12)) ||
-        (t->maxradix_x && (t->maxradix_x < 2 || t->maxradix_x > 16)) || (t->tz && !pow2(t->tz)) ||
+        (t->maxradix_x && (t->maxradix_x < 2 || t->maxradix_x > 18)) || (t->tz && !pow2(t->tz)) ||
         (t->zthreads && (t->zthreads < 32 || t->zthreads > 256)) || (t->xthreads && (t->xthreads < 32 || t->xthreads > 256)) ||
         t->chunk_mb < 0 || t->plane_overlap < 0 || t->plane_overlap > 2)
         return CHAN_EINVAL;
@@ -578,37 +579,28 @@ int chan_step(chan_t* h) {
     return CHAN_OK;
 }
 
-int chan_filter_store(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
-    if (!h || !dev_out) return CHAN_EINVAL;
-    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+}  // extern "C"
+
+namespace {
+
+// the ten output planes of the filter: three velocity copies, then the seven products through the plane kernels
+int filter_args(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes, FieldPtrsW& oF) {
     const Plan& P = h->P;
     if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
-    const size_t per = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1);
-    if (out_bytes < per * 10 * 16) return CHAN_ENOSPACE;
-    double2* out = (double2*)dev_out;
+    const size_t per = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1), esz = h->out_f32 ? 8 : 16;
+    if (out_bytes < per * 10 * esz) return CHAN_ENOSPACE;
+    for (int k = 0; k < 7; ++k) oF.f[k] = (double2*)((char*)dev_out + (size_t)(3 + k) * per * esz);
     PlaneParams Q = pparams(h);
     FieldPtrs in; in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w;
-    PB(CHAN_KC_FILTER_COPY); k_filter_copy<<<296, 256, 0, h->stream>>>(Q, in, out, kxc, kzc); LAUNCHED();
-    FieldPtrsW o;
-    for (int k = 0; k < 7; ++k) o.f[k] = out + (size_t)(3 + k) * per;
-    return run_planes(h, 7, o, kxc, kzc);
+    PB(CHAN_KC_FILTER_COPY); k_filter_copy<<<296, 256, 0, h->stream>>>(Q, in, (double2*)dev_out, kxc, kzc, h->out_f32); LAUNCHED();
+    return CHAN_OK;
 }
 
-int chan_step_filter(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
-    if (!h || !dev_out) return CHAN_EINVAL;
-    if (!h->bound || !h->have_state || h->isub != 0) return CHAN_ESTATE;
-    const Plan& P = h->P;
-    if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
-    const size_t per = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1);
-    if (out_bytes < per * 10 * 16) return CHAN_ENOSPACE;
-    double2* out = (double2*)dev_out;
-    PlaneParams Q = pparams(h);
-    FieldPtrs in; in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w;
-    PB(CHAN_KC_FILTER_COPY); k_filter_copy<<<296, 256, 0, h->stream>>>(Q, in, out, kxc, kzc); LAUNCHED();
+int step_filter_impl(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
     FieldPtrsW oF, oH;
-    for (int k = 0; k < 7; ++k) oF.f[k] = out + (size_t)(3 + k) * per;
-    oH.f[0] = h->H1; oH.f[1] = h->H2; oH.f[2] = h->H3;
     int rc;
+    if ((rc = filter_args(h, kxc, kzc, dev_out, out_bytes, oF))) return rc;
+    oH.f[0] = h->H1; oH.f[1] = h->H2; oH.f[2] = h->H3;
     if ((rc = run_planes_both(h, oH, oF, kxc, kzc))) return rc;
     if ((rc = run_ysolve(h))) return rc;
     h->isub = 1;
@@ -617,12 +609,31 @@ int chan_step_filter(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_byte
     return CHAN_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+int chan_filter_store(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
+    if (!h || !dev_out) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    FieldPtrsW o;
+    int rc = filter_args(h, kxc, kzc, dev_out, out_bytes, o);
+    if (rc) return rc;
+    return run_planes(h, 7, o, kxc, kzc);
+}
+
+int chan_step_filter(chan_t* h, int kxc, int kzc, void* dev_out, size_t out_bytes) {
+    if (!h || !dev_out) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state || h->isub != 0) return CHAN_ESTATE;
+    return step_filter_impl(h, kxc, kzc, dev_out, out_bytes);
+}
+
 int chan_filter_store_host(chan_t* h, int kxc, int kzc, void* host_out, size_t out_bytes) {
     if (!h || !host_out) return CHAN_EINVAL;
     if (!h->bound || !h->have_state) return CHAN_ESTATE;
     const Plan& P = h->P;
     if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
-    const size_t bytes = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1) * 10 * 16;
+    const size_t bytes = (size_t)P.ny * (2 * kzc + 1) * (kxc + 1) * 10 * (h->out_f32 ? 8 : 16);
     if (out_bytes < bytes) return CHAN_ENOSPACE;
     // staged in the y-phase scratch field s1 (idle between substeps): at most one field's worth of output
     if (bytes > h->s1_bytes) return CHAN_ENOSPACE;
@@ -630,6 +641,31 @@ int chan_filter_store_host(chan_t* h, int kxc, int kzc, void* host_out, size_t o
     if (rc) return rc;
     CK(cudaMemcpyAsync(host_out, h->s1, bytes, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
+    return CHAN_OK;
+}
+
+int chan_set_filter_precision(chan_t* h, int bytes_per_real) {
+    if (!h || (bytes_per_real != 4 && bytes_per_real != 8)) return CHAN_EINVAL;
+    h->out_f32 = (bytes_per_real == 4);
+    return CHAN_OK;
+}
+
+int chan_run(chan_t* h, const chan_run_t* r, long long* snapshots) {
+    if (!h || !r) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state || h->isub != 0) return CHAN_ESTATE;
+    if (r->nsteps < 0 || r->filter_every < 0 || r->stats_every < 0) return CHAN_EINVAL;
+    if (r->filter_every > 0 && (!r->dev_ring || r->ring_slots < 1)) return CHAN_EINVAL;
+    long long emitted = 0;
+    for (int n = 0; n < r->nsteps; ++n) {
+        int rc;
+        if (r->stats_every > 0 && n % r->stats_every == 0 && (rc = chan_stats(h, CHAN_STATS_ACCUMULATE, nullptr, nullptr))) return rc;
+        if (r->filter_every > 0 && n % r->filter_every == 0) {
+            char* slot = (char*)r->dev_ring + (size_t)(emitted % r->ring_slots) * r->slot_bytes;
+            if ((rc = step_filter_impl(h, r->kx_cut, r->kz_cut, slot, r->slot_bytes))) return rc;
+            ++emitted;
+        } else if ((rc = chan_step(h))) return rc;
+    }
+    if (snapshots) *snapshots = emitted;
     return CHAN_OK;
 }
 
@@ -767,6 +803,33 @@ int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts) 
             host_ms[h->prof_cls[i]] += ms; host_counts[h->prof_cls[i]] += 1;
         }
     }
+    return CHAN_OK;
+}
+
+int chan_debug_fma_peak(chan_t* h, double* host_tflops) {
+    if (!h || !host_tflops) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * 8, iters = 1 << 16;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {        // first round warms the clocks up
+        CK(cudaEventRecord(e0, h->stream));
+        k_fma_peak<<<blocks, 256, 0, h->stream>>>(h->scal + 7, iters, 0.999999, 1e-9);
+        ++h->launches;
+        CK(cudaEventRecord(e1, h->stream));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        const double tf = 2.0 * 8.0 * iters * (double)blocks * 256.0 / (ms * 1e-3) / 1e12;
+        if (rep && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (!ck(h, cudaGetLastError())) return CHAN_ECUDA;
+    *host_tflops = best;
     return CHAN_OK;
 }
 

@@ -3,7 +3,7 @@
 // ("pseudo-spectral ... fully dealiased by zero padding"), L84 (batched plane FFTs), L124 (filter).
 //
 // Transform engine.  A length-n transform (n = 2^a 3^b) is a list of register-resident stages of radix
-// 2,3,4,6,8,12 (and 16 in the x pass; chan_plan.cpp chooses them), run IN PLACE in shared memory:
+// 2,3,4,6,8,12 (and 16, 18 in the x pass; chan_plan.cpp chooses them), run IN PLACE in shared memory:
 //   spectral -> physical: decimation in frequency, e^{+i}, natural order in, digit-reversed order out;
 //   physical -> spectral: decimation in time, e^{-i}, the same stage list backwards.
 // Physical space is only ever used pointwise, so the digit-reversed order is never undone.
@@ -95,8 +95,37 @@ template <bool INV> CHAN_HD void dft16(c2 (&a)[16]) {
     for (int k1 = 0; k1 < 4; ++k1) { c2 p = y[k1][0], q = y[k1][1], r = y[k1][2], s = y[k1][3]; dft4<INV>(p, q, r, s); a[k1] = p; a[k1 + 4] = q; a[k1 + 8] = r; a[k1 + 12] = s; }
 }
 
+// radix 9 = 3 x 3 (Cooley-Tukey, twiddles w9^(n2 k1)); in natural order, out natural order
+template <bool INV> CHAN_HD void dft9(c2& x0, c2& x1, c2& x2, c2& x3, c2& x4, c2& x5, c2& x6, c2& x7, c2& x8) {
+    const double c1 = 0.76604444311897803520, s1 = 0.64278760968653932632;    // 2 pi/9
+    const double c2_ = 0.17364817766693034885, s2 = 0.98480775301220805937;   // 4 pi/9
+    const double c4 = -0.93969262078590838405, s4 = 0.34202014332566873304;   // 8 pi/9
+    // n = 3 n1 + n2: transforms over n1 for n2 = 0, 1, 2
+    dft3<INV>(x0, x3, x6); dft3<INV>(x1, x4, x7); dft3<INV>(x2, x5, x8);
+    // y[k1][n2] *= w9^(n2 k1):  (k1, n2) = (1,1): x4, (1,2): x5, (2,1): x7, (2,2): x8
+    x4 = mulcs<INV>(x4, c1, s1); x5 = mulcs<INV>(x5, c2_, s2); x7 = mulcs<INV>(x7, c2_, s2); x8 = mulcs<INV>(x8, c4, s4);
+    // X[k1 + 3 k2] = sum over n2 of y[k1][n2] w3^(n2 k2)
+    dft3<INV>(x0, x1, x2); dft3<INV>(x3, x4, x5); dft3<INV>(x6, x7, x8);
+    // now x0,x1,x2 = X[0],X[3],X[6]; x3,x4,x5 = X[1],X[4],X[7]; x6,x7,x8 = X[2],X[5],X[8]: back to natural order
+    const c2 t1 = x1, t2 = x2, t3 = x3, t5 = x5, t6 = x6, t7 = x7;
+    x1 = t3; x2 = t6; x3 = t1; x5 = t7; x6 = t2; x7 = t5;
+}
+// radix 18 = 2 x 9 by the prime-factor map n = (9 n1 + 2 n2) mod 18, k = (9 k1 + 10 k2) mod 18: no internal twiddles
+template <bool INV> CHAN_HD void dft18(c2 (&a)[18]) {
+    c2 e0 = a[0], e1 = a[2], e2 = a[4], e3 = a[6], e4 = a[8], e5 = a[10], e6 = a[12], e7 = a[14], e8 = a[16];      // n1 = 0
+    c2 o0 = a[9], o1 = a[11], o2 = a[13], o3 = a[15], o4 = a[17], o5 = a[1], o6 = a[3], o7 = a[5], o8 = a[7];      // n1 = 1
+    dft9<INV>(e0, e1, e2, e3, e4, e5, e6, e7, e8);
+    dft9<INV>(o0, o1, o2, o3, o4, o5, o6, o7, o8);
+    // k1 = 0 -> k = (10 k2) mod 18 = 0,10,2,12,4,14,6,16,8;  k1 = 1 -> k = (9 + 10 k2) mod 18 = 9,1,11,3,13,5,15,7,17
+    a[0] = e0 + o0; a[9] = e0 - o0; a[10] = e1 + o1; a[1] = e1 - o1; a[2] = e2 + o2; a[11] = e2 - o2;
+    a[12] = e3 + o3; a[3] = e3 - o3; a[4] = e4 + o4; a[13] = e4 - o4; a[14] = e5 + o5; a[5] = e5 - o5;
+    a[6] = e6 + o6; a[15] = e6 - o6; a[16] = e7 + o7; a[7] = e7 - o7; a[8] = e8 + o8; a[17] = e8 - o8;
+}
+
 template <int R, bool INV> CHAN_HD void bfly(c2 (&a)[R]) {
-    if constexpr (R == 16) {
+    if constexpr (R == 18) {
+        dft18<INV>(a);
+    } else if constexpr (R == 16) {
         dft16<INV>(a);
     } else if constexpr (R == 2) {
         dft2<INV>(a[0], a[1]);
@@ -149,7 +178,7 @@ template <int R, bool INV> CHAN_HD void bfly(c2 (&a)[R]) {
 template <int R>
 CHAN_HD void load_twiddles(const FftStage& S, int m, int p, c2 (&tw)[R - 1 > 0 ? R - 1 : 1]) {
     if constexpr (R > 12) {
-        tw[0] = ldtw(S.tw + p);         // radix 16: pass_item forms w^k on the fly (a register file of 15 powers would spill)
+        tw[0] = ldtw(S.tw + p);         // radix 16, 18: pass_item forms w^k on the fly (a register file of 15 or 17 powers would spill)
     } else if constexpr (R >= 2) {
 #if CHAN_TW_POWERS
         tw[0] = ldtw(S.tw + p);
@@ -269,7 +298,7 @@ CHAN_HD void zinv_phase(int ph, int tid, int nt, const PlaneParams& P, int T, c2
 
 // ---- K4 (a7-a8): forward c2c along z, truncate, scale ----------------------------------------------
 //   filt 0: retained modes into plane-layout fields (Nyquist slot zeroed), all p < pin = nxh;
-//   filt 1: |q| <= kzc, p <= kxc into out[j][2kzc+1][kxc+1].
+//   filt 1: |q| <= kzc, p <= kxc into out[j][2kzc+1][kxc+1] (complex128);  filt 2: the same as complex64.
 // in: xh[f][jc][r][pin].
 struct ZFwdIO {
     c2* sm; int T;
@@ -293,7 +322,10 @@ struct ZFwdIO {
             const int nr = 2 * kzc + 1, npk = kxc + 1;
             int rr;
             if (e <= kzc) rr = e; else if (e >= mz - kzc) rr = e - mz + nr; else return;
-            if (p0 + t < npk) ststream(dst + (size_t)rr * npk + p0 + t, mk(v.x * scale, v.y * scale));
+            if (p0 + t >= npk) return;
+            if (filt == 1) ststream(dst + (size_t)rr * npk + p0 + t, mk(v.x * scale, v.y * scale));
+            else           // filt 2: the database in binary32, rounded once (to nearest even) from the fp64 result
+                reinterpret_cast<float2*>(dst)[(size_t)rr * npk + p0 + t] = make_float2((float)(v.x * scale), (float)(v.y * scale));
         }
     }
 };
@@ -310,6 +342,13 @@ CHAN_HD void zfwd_phase(int ph, int tid, int nt, const PlaneParams& P, int T, c2
 // Kernels.  k_z*_g: any stage list (run-time radix switch; correct for every 2^a 3^b length but the
 // compiler keeps the registers of all radices alive).  k_z*_s<R0..R3>: the same phases with the stage
 // radices as template parameters (R = 1: absent) -- the plans chan_api.cu dispatches to.
+// plane j of an output field of the forward z pass: full field (filt 0), filtered complex128 (1) or complex64 (2)
+CHAN_HD double2* zfwd_plane(const PlaneParams& P, double2* f, int j, int filt, int kxc, int kzc) {
+    const size_t per = (size_t)(2 * kzc + 1) * (kxc + 1);
+    if (filt == 0) return f + (size_t)j * P.nm;
+    if (filt == 1) return f + (size_t)j * per;
+    return reinterpret_cast<double2*>(reinterpret_cast<float2*>(f) + (size_t)j * per);
+}
 CHAN_HD ZInvIO make_zinv_io(const PlaneParams& P, int T, c2* sm, const double2* src, double2* dst, int p0) {
     ZInvIO io;
     io.sm = sm; io.T = T; io.gin = false; io.gout = false;
@@ -349,7 +388,7 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_g(CHAN_ZARGS_FWD) {
     const int p0 = blockIdx.x * T, jc = blockIdx.y, fi = blockIdx.z;
     const int j = j0 + jc;
     const double2* src = xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin;
-    double2* dst = filt ? out.f[fi] + (size_t)j * (2 * kzc + 1) * (kxc + 1) : out.f[fi] + (size_t)j * P.nm;
+    double2* dst = zfwd_plane(P, out.f[fi], j, filt, kxc, kzc);
 #pragma unroll 1
     for (int ph = 0; ph < P.fz.ns; ++ph) {
         if (ph) __syncthreads();
@@ -393,8 +432,7 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
     const int p0 = bx * T;
     const int j = j0 + jc;
     ZFwdIO io = make_zfwd_io(P, T, reinterpret_cast<c2*>(smem_raw), xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin,
-                             filt ? out.f[fi] + (size_t)j * (2 * kzc + 1) * (kxc + 1) : out.f[fi] + (size_t)j * P.nm, pin, p0, scale,
-                             filt, kxc, kzc);
+                             zfwd_plane(P, out.f[fi], j, filt, kxc, kzc), pin, p0, scale, filt, kxc, kzc);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true;
@@ -450,11 +488,25 @@ struct XIO {
 template <int R, bool INV, bool DIT, int M = 0>
 CHAN_HD void xpass(const XIO& io, const FftStage& S, int n, int nseq, int tid, int nt) {
     const int m = M > 0 ? M : S.m, ncur = R * m, nb = n / R;
-    for (int b = tid; b < nb; b += nt) {
-        const int blk = b / m, p = b - blk * m;
-        c2 tw[R - 1 > 0 ? R - 1 : 1];
-        if (m > 1) load_twiddles<R>(S, m, p, tw);
-        for (int q = 0; q < nseq; ++q) pass_item<R, INV, DIT>(io, io, q, blk * ncur + p, m, tw, m > 1);
+    if constexpr (R > 12) {
+        // radix 16, 18: a row has fewer butterflies than the CTA has threads, and 2R doubles of butterfly data leave no
+        // room to interleave sequences: work item = (sequence, butterfly), one sequence at a time per thread
+        const int total = nb * nseq;
+#pragma unroll 1
+        for (int w = tid; w < total; w += nt) {
+            const int q = w / nb, b = w - q * nb;
+            const int blk = b / m, p = b - blk * m;
+            c2 tw[R - 1];
+            if (m > 1) load_twiddles<R>(S, m, p, tw);
+            pass_item<R, INV, DIT>(io, io, q, blk * ncur + p, m, tw, m > 1);
+        }
+    } else {
+        for (int b = tid; b < nb; b += nt) {
+            const int blk = b / m, p = b - blk * m;
+            c2 tw[R - 1 > 0 ? R - 1 : 1];
+            if (m > 1) load_twiddles<R>(S, m, p, tw);
+            for (int q = 0; q < nseq; ++q) pass_item<R, INV, DIT>(io, io, q, blk * ncur + p, m, tw, m > 1);
+        }
     }
 }
 template <bool INV, bool DIT>
@@ -466,6 +518,7 @@ CHAN_HD void xpass_any(const XIO& io, const FftStage& S, int n, int nseq, int ti
         case 6: xpass<6, INV, DIT>(io, S, n, nseq, tid, nt); break;
         case 8: xpass<8, INV, DIT>(io, S, n, nseq, tid, nt); break;
         case 16: xpass<16, INV, DIT>(io, S, n, nseq, tid, nt); break;
+        case 18: xpass<18, INV, DIT>(io, S, n, nseq, tid, nt); break;
         default: xpass<12, INV, DIT>(io, S, n, nseq, tid, nt); break;
     }
 }

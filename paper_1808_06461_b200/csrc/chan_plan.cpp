@@ -166,10 +166,10 @@ void pad8(int ny, const std::vector<double>& T, std::vector<double>& O) {
 
 // Stage list for length n = 2^a 3^b (chan_fft.cuh).  `fused_last` > 0 fixes the last radix (the x
 // transform fuses that stage with the pointwise products); the rest is the shortest list of radices from
-// {16,12,8,6,4,3,2} (fewest radix-12/16 stages among the shortest), radices with a factor 3 first so that the
+// {18,16,12,8,6,4,3,2} (fewest radix-12/16 stages among the shortest), radices with a factor 3 first so that the
 // zero band of the 3/2 padding lines up with whole inputs of the first butterfly.
 void best_radices(int rest, int maxr, std::vector<int>& cur, std::vector<int>& best) {
-    static const int cand[7] = {16, 12, 8, 6, 4, 3, 2};
+    static const int cand[8] = {18, 16, 12, 8, 6, 4, 3, 2};
     if (rest == 1) {
         auto key = [](const std::vector<int>& v) {
             int big = 0, c2 = 0, mx = 0;
@@ -237,11 +237,11 @@ bool make_fft_plan(int n, int fused_last, int maxr, FftPlan& F) {
 
 // Stage lists of the two transform lengths.  xfuse: 4 | 8 = radix of the x stage fused with the products (0: the one
 // that gives the shorter stage list, then the one without radix-12 stages, then 4: lighter fused stage);
-// maxr: largest radix of a z stage (0: 12); maxrx: largest radix of an x stage (0: 16 -- two shared-memory stages in
-// front of the fused one at 1536 points).
+// maxr: largest radix of a z stage (0: 12); maxrx: largest radix of an x stage (0: 18 -- two shared-memory stages in
+// front of the fused one at 1536 points [12,16|8] and at 2304 points [18,16|8]).
 int plan_ffts(Plan& P, int xfuse, int maxr, int maxrx) {
     if (maxr < 2) maxr = 12;
-    if (maxrx < 2) maxrx = 16;
+    if (maxrx < 2) maxrx = 18;
     int fuse = 4;
     if (xfuse == 4 || xfuse == 8) fuse = xfuse;
     else {

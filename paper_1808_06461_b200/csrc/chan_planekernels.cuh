@@ -11,7 +11,7 @@ namespace chn {
 // =====================================================================================================
 // a13 first part: copy the retained modes of u,v,w (plane layout) into the filter output.
 // =====================================================================================================
-__global__ void k_filter_copy(PlaneParams P, FieldPtrs in, double2* __restrict__ out, int kxc, int kzc) {
+__global__ void k_filter_copy(PlaneParams P, FieldPtrs in, double2* __restrict__ out, int kxc, int kzc, int f32) {
     const int nr = 2 * kzc + 1, npk = kxc + 1;
     const size_t per = (size_t)P.ny * nr * npk;
     const size_t total = 3 * per;
@@ -22,7 +22,9 @@ __global__ void k_filter_copy(PlaneParams P, FieldPtrs in, double2* __restrict__
         rem -= (size_t)j * nr * npk;
         const int rr = (int)(rem / npk), p = (int)(rem - (size_t)rr * npk);
         const int s = (rr <= kzc) ? rr : P.nz - (nr - rr);
-        out[w] = in.f[fi][(size_t)j * P.nm + (size_t)s * P.nxh + p];
+        const double2 val = in.f[fi][(size_t)j * P.nm + (size_t)s * P.nxh + p];
+        if (!f32) out[w] = val;
+        else reinterpret_cast<float2*>(out)[w] = make_float2((float)val.x, (float)val.y);   // binary32 database: round to nearest even
     }
 }
 
@@ -87,6 +89,22 @@ __global__ void __launch_bounds__(256) k_transpose(const double2* __restrict__ i
         const long long c = c0 + k, r = r0 + tx;
         if (r < R && c < C) out[c * R + r] = tile[tx][k];
     }
+}
+
+// =====================================================================================================
+// fp64 FMA micro-benchmark (bench.py's "alu" roof): 8 independent register-only DFMA chains per
+// thread, `iters` rounds; nothing touches memory until the final store that keeps the chains alive.
+// flops = 2 * 8 * iters * threads.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) k_fma_peak(double* __restrict__ sink, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+#pragma unroll 4
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 12345.678) sink[0] = s;      // practically never: the store only pins the arithmetic
 }
 
 }  // namespace chn

@@ -78,3 +78,56 @@ def test_stats_accumulate_read_reset():
     assert np.all(s[3] >= 0) and np.all(s[6] >= 0) and np.all(s[8] >= 0) and np.all(s[9] >= 0)
     o.stats_reset()
     assert o.stats_read()[1] == 0 and not o.stats_read()[0].any()
+
+
+def test_single_precision_database_is_the_fp64_database_rounded_once_to_nearest_even():
+    """NEXT-1 (the stored values take about four bytes each): filter_store(single=True) must be the
+    fp64 database -- pinned by the tests above -- rounded once per component to binary32, ties to even.  The rounding
+    is re-derived here from the bit pattern of the double (integer arithmetic on the mantissa), not by calling the
+    cast again; mode selection is untouched (same shape, zeros stay zeros)."""
+    c, o = _setup()
+    d64 = o.filter_store(*c["cut"])
+    d32 = o.filter_store(*c["cut"], single=True)
+    assert d32.dtype == np.complex64 and d32.shape == d64.shape
+
+    def round_to_f32_bits(x):
+        """IEEE round-to-nearest-even of positive normal doubles to binary32, from the bits."""
+        b = np.abs(x).view(np.uint64)
+        e = ((b >> np.uint64(52)) & np.uint64(0x7FF)).astype(np.int64) - 1023
+        m = (b & np.uint64((1 << 52) - 1)) | np.uint64(1 << 52)                 # 53-bit significand
+        keep, rest = m >> np.uint64(29), m & np.uint64((1 << 29) - 1)           # 24 bits kept, 29 dropped
+        half = np.uint64(1 << 28)
+        up = (rest > half) | ((rest == half) & ((keep & np.uint64(1)) == 1))
+        keep = keep + up.astype(np.uint64)
+        val = keep.astype(np.float64) * np.exp2((e - 23).astype(np.float64))     # exact: 25 bits times a power of two
+        return np.sign(x) * val
+
+    for part in (np.real, np.imag):
+        x = part(d64).ravel()
+        y = part(d32).ravel().astype(np.float64)
+        normal = (np.abs(x) > 1e-30) & (np.abs(x) < 1e30)                      # binary32 normal range, far from its ends
+        assert normal.sum() > 0.5 * x.size
+        assert np.array_equal(y[normal], round_to_f32_bits(x[normal]))
+        assert np.array_equal(y[x == 0.0], x[x == 0.0])
+        assert np.abs(y[normal] - x[normal]).max() <= 2.0 ** -24 * np.abs(x[normal]).max()
+    # ties go to even: 1 + 2^-24 -> 1, 1 + 3 * 2^-24 -> 1 + 2^-22 (hand values through the same helper and the cast)
+    t = np.array([1.0 + 2.0 ** -24, 1.0 + 3.0 * 2.0 ** -24, 1.0 + 2.0 ** -24 + 2.0 ** -50])
+    assert np.array_equal(round_to_f32_bits(t), np.array([1.0, 1.0 + 2.0 ** -22, 1.0 + 2.0 ** -23]))
+    assert np.array_equal(t.astype(np.float32).astype(np.float64), round_to_f32_bits(t))
+
+
+def test_run_emits_snapshots_at_the_cadence():
+    """oracle.run == the plain loop of filter_store / stats_accumulate / step written out (L110-112)."""
+    c, o = _setup()
+    c2, ref = _setup()
+    snaps = o.run(5, 2, 1, *c["cut"], single=True)
+    want = []
+    for n in range(5):
+        ref.stats_accumulate()
+        if n in (0, 2, 4):
+            want.append(ref.filter_store(*c["cut"], single=True))
+        ref.step()
+    assert len(snaps) == 3 and all(np.array_equal(a, b) for a, b in zip(snaps, want))
+    assert np.array_equal(o.stats_read()[0], ref.stats_read()[0]) and o.stats_read()[1] == 5
+    assert np.array_equal(o.v, ref.v)
+    assert o.run(2, 0, 0, *c["cut"]) == []
