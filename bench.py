@@ -48,11 +48,33 @@ SURVEY_GROUPS = {
 }
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the ncu --set full capture
-# of profiles/r1f_summary.md (not measured live): keyed by (class, mx, mz, planes per launch).
-NCU_TRAFFIC = {("xfft_prod", 2304, 1728, 11): 1.401605e9 + 0.661527e9, ("zfft_inv", 2304, 1728, 11): 0.933496e9 + 1.371144e9,
-               ("zfft_fwd", 2304, 1728, 11): 0.700743e9 + 0.439941e9}
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 fp64 FMA/clk x 2 x 1965 MHz
+# Per-launch hardware counters of the hot kernels come from the committed `ncu --set full` table of THIS round
+# (profiles/r2_summary.md names the command): roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum, and the
+# shared-memory roof uses l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.  They are not measured live (a number taken
+# under a profiler is never a bench value): the JSON says which file and row they come from, and they are null when
+# the table has no launch of the same kernel with the same grid.
+NCU_TABLE = os.path.join("profiles", "r2_ncu_full_cfg5slab.csv")
+KERNEL_OF_CLASS = {"xfft_prod": "k_xfft_prod_s<3", "xfft_prod_filter": "k_xfft_prod_s<7", "zfft_inv": "k_zfft_inv_s", "zfft_fwd": "k_zfft_fwd_s",
+                   "planes_merged": "k_planes_s", "y1": "k_sa(", "y2": "k_sb(", "y3": "k_sc(", "y4": "k_sd(", "derive_down": "k_se(",
+                   "derive_up": "k_sf(", "stats": "k_stats("}
+FP64_PEAK_DERIVED_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 fp64 FMA/clk x 2 x 1965 MHz (guide's unit counts): a note beside the measured peak
+SMEM_BYTES_PER_CLK_PER_SM = 128                              # one 128-byte shared-memory wavefront per clock per SM
+
+
+def ncu_row(cls, grid):
+    """Row of the committed ncu table for kernel class `cls` launched with `grid` (tuple), or None."""
+    import csv
+    path = os.path.join(ROOT, NCU_TABLE)
+    name = KERNEL_OF_CLASS.get(cls)
+    if not name or not os.path.exists(path):
+        return None
+    with open(path, newline="") as fh:
+        rows = list(csv.DictReader(fh))
+    want = "(" + ", ".join(str(int(g)) for g in grid) + ")"
+    for r in rows:
+        if name in (r.get("Kernel Name") or "") and (r.get("Grid Size") or "").replace(" ", "") == want.replace(" ", ""):
+            return r
+    return None
 
 
 def xpass_flops_per_point(nx, nz):
@@ -165,6 +187,46 @@ def oracle_sample(cfg_name, steps, warmup):
     sample = (f"oracle.ChannelOracle, {steps} x (step + filter_store + stats) on a {snx}x{cs['ny']}x{snz} sub-box of {cfg_name} "
               f"(same mesh, Re, dt, dx, dz; {pts} points)")
     return 3 * pts * steps / dt / 1e6, dt / steps * 1e3, sample
+
+
+def _oracle_worker(cfg_name, barrier, q):
+    """One process of the all-core baseline: builds its oracle, waits for the others, runs one sample step."""
+    import numpy  # noqa: F401  (spawned: fresh interpreter)
+    os.environ.setdefault("OMP_NUM_THREADS", "1")
+    from oracle.channel import ChannelOracle
+    from paper_1808_06461_b200 import inputs
+    c = inputs.config(cfg_name)
+    snx, snz = min(c["nx"], 48), min(c["nz"], 32)
+    cs = inputs.config(cfg_name, nx=snx, nz=snz, lx=c["lx"] * snx / c["nx"], lz=c["lz"] * snz / c["nz"],
+                       cut=(min(c["cut"][0], snx // 2 - 1), min(c["cut"][1], snz // 2 - 1)))
+    v, phi, omy = (t.numpy() for t in inputs.fluctuations(cs))
+    o = ChannelOracle(cs["nx"], cs["ny"], cs["nz"], cs["lx"], cs["lz"], cs["y"], cs["re"], cs["dt"])
+    o.set_state(v, phi, omy, cs["U"], cs["W"])
+    barrier.wait(timeout=600)
+    t0 = time.perf_counter()
+    o.step()
+    o.filter_store(*cs["cut"])
+    o.stats_accumulate()
+    q.put((cs["nx"] * cs["ny"] * cs["nz"], t0, time.perf_counter()))
+
+
+def oracle_all_cores(cfg_name, ncores):
+    """The oracle as it stands on every host core at once: one independent sub-box per core (the oracle itself is
+    single-threaded numpy; the wall-normal stages are independent per mode, so a slab of modes per core is how it
+    would be spread), all started together; value = all points x 3 substeps / (last finish - first start)."""
+    import multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    bar, q = ctx.Barrier(ncores), ctx.Queue()
+    procs = [ctx.Process(target=_oracle_worker, args=(cfg_name, bar, q)) for _ in range(ncores)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=700) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+    wall = max(r[2] for r in res) - min(r[1] for r in res)
+    pts = sum(r[0] for r in res)
+    return 3 * pts / wall / 1e6, (f"{ncores} processes x (step + filter_store + stats) of oracle.ChannelOracle, one 48 x ny x 32 sub-box of "
+                                  f"{cfg_name} each, started together; {pts} points in {wall:.1f} s")
 
 
 def cufft_reference_line(c, dev, npl=8):
@@ -357,16 +419,35 @@ def main():
     abytes = BYTES_PER_POINT[dom] * pts_per_launch
     achieved = abytes / (dms / dcnt * 1e-3) / 1e9
     planes_per_launch = round(pts_per_launch / (c["nx"] * c["nz"]))
+    mz_, tiles_ = 3 * c["nz"] // 2, -(-(c["nx"] // 2) // tune["tz"])
+    grid = {"xfft_prod": (mz_, planes_per_launch, 1), "zfft_inv": (tiles_, planes_per_launch, 6), "zfft_fwd": (tiles_, planes_per_launch, 3)}.get(dom)
+    row = ncu_row(dom, grid) if grid else None
+    traffic = (float(row["dram__bytes_read.sum"]) + float(row["dram__bytes_write.sum"])) * 1e9 if row else None
     roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC.get((dom, 3 * c["nx"] // 2, 3 * c["nz"] // 2, planes_per_launch)),
+                "traffic": traffic,
+                "traffic_source": (f"{NCU_TABLE}, row of {row['Kernel Name'][:40]}... grid {row['Grid Size']} (ncu --set full capture of "
+                                   "this round, not measured in this run)") if row else "no matching launch in " + NCU_TABLE,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
                 "avg_launch_ms": dms / dcnt, "share_of_step": dms / ms_total}
     if dom == "xfft_prod":
-        # the x pass is bound by shared memory and the fp64 pipe, not by HBM (profiles/r1e_summary.md): second roof
+        # the x pass is bound by the shared-memory pipe and the fp64 pipe, not by HBM: two more
+        # roofs.  "alu": 5 N log2 N flops against the fp64 FMA rate measured by the library's register-only micro-kernel
+        # (chan_debug_fma_peak) in this run; "smem": shared-memory wavefronts of one launch (ncu table) x 128 B against
+        # 148 SMs x 128 B/clk x the SM clock sampled during the timed region.
         fl = xpass_flops_per_point(c["nx"], c["nz"]) * pts_per_launch
         tf = fl / (dms / dcnt * 1e-3) / 1e12
-        roofline["fp64"] = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
-                            "flops_per_launch": fl, "peak_source": "derived: 148 SM x 64 FMA/clk x 2 x 1.965 GHz"}
+        fma_peak = ch.debug_fma_peak()
+        roofline["fp64"] = {"bound": "alu", "achieved": tf, "peak": fma_peak, "unit": "TFLOP/s", "frac": tf / fma_peak, "flops_per_launch": fl,
+                            "peak_source": "measured: chan_debug_fma_peak (8 independent DFMA chains per thread, 8 CTAs of 256 threads per SM)",
+                            "peak_derived_note": FP64_PEAK_DERIVED_TFLOPS}
+        clk_mhz = clk.summary().get("sm_mhz") or 1965.0
+        if row and row.get("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum"):
+            wf = float(row["l1tex__data_pipe_lsu_wavefronts_mem_shared.sum"])
+            sm_peak = 148 * SMEM_BYTES_PER_CLK_PER_SM * clk_mhz * 1e6 / 1e9
+            sm_ach = wf * 128 / (dms / dcnt * 1e-3) / 1e9
+            roofline["smem"] = {"bound": "smem", "achieved": sm_ach, "peak": sm_peak, "unit": "GB/s", "frac": sm_ach / sm_peak,
+                                "wavefronts_per_launch": wf, "peak_source": f"148 SMs x 128 B/clk x {clk_mhz:.0f} MHz (sampled)",
+                                "wavefront_source": NCU_TABLE}
     groups = {}
     for gname, (classes, bpp) in SURVEY_GROUPS.items():
         if merged and gname.startswith(("K2 ", "K3 ", "K4 ")):
@@ -433,9 +514,14 @@ def main():
             cufft = {"error": str(ex)[:200]}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
+        ncores = len(os.sched_getaffinity(0))
         val, ms, sample = oracle_sample(wl, 1, 0)
-        cpu = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-               "host_cores_available": len(os.sched_getaffinity(0))}
+        cpu = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "host_cores_available": ncores}
+        try:
+            allv, alls = oracle_all_cores(wl, ncores)
+            cpu["all_cores"] = {"value": allv, "unit": UNIT, "cores": ncores, "sample": alls}
+        except Exception as ex:                    # the baseline is context: never fail the bench line over it
+            cpu["all_cores"] = {"value": None, "error": str(ex)[:200]}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,

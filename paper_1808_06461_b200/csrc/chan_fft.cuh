@@ -571,12 +571,30 @@ CHAN_HD void xfused(const XIO& io, int n, int tid, int nt) {
 }
 
 CHAN_HD void xpack(const XIO& io, int mx, int nxh, const double2* zrow, size_t fstride, int tid, int nt, bool fill_zero) {
-    // C[k] = A[k] + i B[k], C[mx-k] = conj(A[k]) + i conj(B[k]); Im of the k = 0 entries dropped (R14)
-    for (int w = tid; w < 3 * nxh; w += nt) {
-        const int pr = w / nxh, k = w - pr * nxh;
-        const c2 A = ldstream(zrow + (size_t)(2 * pr) * fstride + k), B = ldstream(zrow + (size_t)(2 * pr + 1) * fstride + k);
-        if (k == 0) io.store(0, pr, mk(A.x, B.x));
-        else { io.store(k, pr, mk(A.x - B.y, A.y + B.x)); io.store(mx - k, pr, mk(A.x + B.y, -A.y + B.x)); }
+    // C[k] = A[k] + i B[k], C[mx-k] = conj(A[k]) + i conj(B[k]); Im of the k = 0 entries dropped (R14).
+    // The global loads of XB work items are issued before the first shared-memory store: one exposed memory latency
+    // per XB items instead of one per item (a 768-column row is 9 items per thread at 256 threads).
+    constexpr int XB = 5;
+    const int total = 3 * nxh;
+    for (int w0 = tid; w0 < total; w0 += nt * XB) {
+        c2 A[XB], B[XB];
+#pragma unroll
+        for (int i = 0; i < XB; ++i) {
+            const int w = w0 + i * nt;
+            if (w < total) {
+                const int pr = w / nxh, k = w - pr * nxh;
+                A[i] = ldstream(zrow + (size_t)(2 * pr) * fstride + k); B[i] = ldstream(zrow + (size_t)(2 * pr + 1) * fstride + k);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < XB; ++i) {
+            const int w = w0 + i * nt;
+            if (w < total) {
+                const int pr = w / nxh, k = w - pr * nxh;
+                if (k == 0) io.store(0, pr, mk(A[i].x, B[i].x));
+                else { io.store(k, pr, mk(A[i].x - B[i].y, A[i].y + B[i].x)); io.store(mx - k, pr, mk(A[i].x + B[i].y, -A[i].y + B[i].x)); }
+            }
+        }
     }
     const int nzero = fill_zero ? mx - 2 * nxh + 1 : 0;     // entries nxh .. mx-nxh (else the first stage reads them as zero)
     for (int w = tid; w < 3 * nzero; w += nt) {

@@ -54,6 +54,7 @@ def seeded_state(c, boost=1.0):
 K_FLOOR = 4.0
 # the same per (kx,kz) line, so that low-energy modes are checked and not hidden in the whole-field norm
 K_LINE = 16.0
+ABS_LINE = 1e-11
 
 
 def make_hp(o):
@@ -89,6 +90,12 @@ def check_lines(gpu, o, h, nsub, where):
         if not live.any():
             continue
         bound = np.maximum(TOL_SUBSTEP * nsub, K_LINE * np.maximum(f, np.median(f[live])))
+        # weak lines: transform roundoff leaks eps x (strongest modes) into every mode (the oracle's own absolute error
+        # on config 1's weak lines is up to 8e-12 of the strongest line, the kernels' -- twiddles by products, a few
+        # ulp -- about twice that on some): an ABSOLUTE error below ABS_LINE = 1e-11 x the strongest line is within
+        # north_star's tolerance whatever it is relative to a line 1e-8 times weaker
+        nrm = np.linalg.norm(ref, axis=-1)
+        bound = np.maximum(bound, ABS_LINE * nrm.max() / np.where(nrm > 0, nrm, 1.0))
         ratio = np.where(live, e / bound, 0.0)
         worst[k] = float(ratio.max())
         idx = np.unravel_index(np.argmax(ratio), ratio.shape)
@@ -496,12 +503,12 @@ def test_step_filter_is_filter_store_then_step_bit_for_bit(B, name):
         assert torch.equal(a, b)
 
 
-@pytest.mark.parametrize("name,chunk_mb", [("mid", 4), ("cfg1", 0)])
+@pytest.mark.parametrize("name,chunk_mb", [("mid", 3), ("cfg1", 0)])
 def test_merged_plane_launches_equal_separate_launches(B, name, chunk_mb):
     """chan_tuning_t.plane_overlap: launch t of the merged kernel carries the inverse z pass of plane chunk t, the x pass
     of chunk t-1 and the forward z pass of chunk t-2 on double-buffered chunk buffers; the planes are independent, so
-    the result must not depend on the launch structure or on the chunk size beyond rounding ("mid" with 4 MiB chunks:
-    22 chunks of 3 planes with a ragged last one against 13 chunks of 5)."""
+    the result must not depend on the launch structure or on the chunk size beyond rounding ("mid" with 3 MiB chunks:
+    33 chunks of 2 planes against 17 chunks of 4, both with a ragged last one)."""
     c = inputs.config(name)
     v, phi, omy = seeded_state(c, 20.0 if name == "cfg1" else 1.0)
     res = []
