@@ -126,6 +126,27 @@ typedef struct {
 } chan_run_t;
 int chan_run(chan_t* h, const chan_run_t* r, long long* snapshots);
 
+/* ---- post-processing of a stored database (NEXT-2; section 3.2) ---------------------------
+ * dev_db is a complex128 database as written by chan_filter_store / chan_step_filter / chan_run with the same
+ * cutoffs, [10][ny][2 kz_cut+1][kx_cut+1].  The handle supplies the mesh, its compact operators, nu and the box; it
+ * may be the handle that produced the database or any other handle on the same mesh and box whose retained modes
+ * contain the stored ones -- typically a small one on the storage grid (nx >= 2 kx_cut + 2, nz >= 2 kz_cut + 2), which
+ * is what post-processing the stored data offline amounts to.  dev_scratch: caller-owned device memory of at least
+ * chan_post_scratch_bytes() bytes (CHAN_ENOSPACE otherwise).  Outputs are complex128 planes [ny][2 kz_cut+1][kx_cut+1]
+ * in the database's mode order.  Asynchronous on the bound stream.  Readings R17-R20 of DESIGN.md. */
+size_t chan_post_scratch_bytes(const chan_t* h, int kx_cut, int kz_cut);
+/* Filtered pressure from the Poisson equation (3.2) d_kk p = -d_ij(u_i u_j) (L126-132) with the Neumann data of a
+ * no-slip wall d_y p = nu d_yy v taken from the stored v (R18), solved per mode with the substep's compact operators
+ * and wall superposition (R19); mode (0,0): p = -(vv) + (vv)(-1). */
+int chan_post_pressure(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* dev_p, void* dev_scratch, size_t scratch_bytes);
+/* Filtered S_ij S_ij = d_ij(u_i u_j) + om_i om_i / 2: identity (3.3) of L134 as re-derived in reading R17. */
+int chan_post_strain_norm(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* dev_out, void* dev_scratch, size_t scratch_bytes);
+/* Sub-grid stresses (3.4), L149: dev_tau[6][ny][2 kz_cut+1][kx_cut+1] = stored u_i u_j minus the product of the STORED
+ * velocities, formed by the library's dealiased product path on this handle's grid and pruned to the cutoff (R20),
+ * order uu,uv,uw,vv,vw,ww.  Overwrites the handle's derived fields u, w, om_x, om_z and rebuilds them (step a1) if the
+ * handle has a state; CHAN_ESTATE mid-step. */
+int chan_post_sgs(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* dev_tau, void* dev_scratch, size_t scratch_bytes);
+
 /* Plane statistics (a14; "Regular statistics of the fully resolved flow are computed and stored
  * on-the-fly"; the profiles are those of the ten variables of L124): flags is an OR of the values below.  ACCUMULATE adds the ten profiles
  * <u>,<v>,<w>,<uu>,<uv>,<uw>,<vv>,<vw>,<ww>,<om_i om_i> of the current state to the running sums;
@@ -191,7 +212,7 @@ long long chan_debug_launch_count(const chan_t* h);
 enum { CHAN_KC_D1FWD = 0, CHAN_KC_DERIVE_DOWN, CHAN_KC_DERIVE_UP, CHAN_KC_ZFFT_INV, CHAN_KC_XFFT_PROD, CHAN_KC_ZFFT_FWD,
        CHAN_KC_MEAN, CHAN_KC_Y1, CHAN_KC_Y2, CHAN_KC_Y3, CHAN_KC_Y4, CHAN_KC_Y5, CHAN_KC_TRANSPOSE,
        CHAN_KC_FILTER_COPY, CHAN_KC_XFFT_PROD_FILTER, CHAN_KC_ZFFT_FWD_FILTER, CHAN_KC_STATS, CHAN_KC_PLANES_MERGED,
-       CHAN_KC_COUNT };
+       CHAN_KC_POST, CHAN_KC_COUNT };
 int chan_debug_profile(chan_t* h, int enable);
 int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts);
 /* fp64 FMA throughput of the device, measured with a register-only micro-kernel (8 independent DFMA chains per thread,

@@ -25,9 +25,10 @@ EXPORTS = [
     "chan_debug_get_field", "chan_debug_set_field", "chan_debug_run_stage", "chan_debug_set_substep_index",
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
     "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe", "chan_debug_fma_peak", "chan_set_filter_precision", "chan_run",
+    "chan_post_scratch_bytes", "chan_post_pressure", "chan_post_strain_norm", "chan_post_sgs",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
-                  "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged"]
+                  "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged", "post"]
 
 
 class Grid(C.Structure):
@@ -105,6 +106,10 @@ def load():
         "chan_debug_fma_peak": (i, [vp, C.POINTER(C.c_double)]),
         "chan_set_filter_precision": (i, [vp, i]),
         "chan_run": (i, [vp, C.POINTER(Run), C.POINTER(C.c_longlong)]),
+        "chan_post_scratch_bytes": (sz, [vp, i, i]),
+        "chan_post_pressure": (i, [vp, i, i, vp, vp, vp, sz]),
+        "chan_post_strain_norm": (i, [vp, i, i, vp, vp, vp, sz]),
+        "chan_post_sgs": (i, [vp, i, i, vp, vp, vp, sz]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -246,6 +251,25 @@ class Channel:
         n = C.c_longlong(0)
         _chk(self.lib.chan_run(self.h, C.byref(r), C.byref(n)), "chan_run")
         return ring, int(n.value)
+
+    # ---- post-processing of a stored database (NEXT-2) ----------------------------------------------
+    def _post(self, fn, name, kx_cut, kz_cut, db, lead=()):
+        assert db.dtype == torch.complex128 and db.is_contiguous() and tuple(db.shape) == (10, self.ny, 2 * kz_cut + 1, kx_cut + 1)
+        out = torch.empty(tuple(lead) + (self.ny, 2 * kz_cut + 1, kx_cut + 1), dtype=torch.complex128, device=self.device)
+        n = int(self.lib.chan_post_scratch_bytes(self.h, kx_cut, kz_cut))
+        scratch = torch.empty(max(n, 16), dtype=torch.uint8, device=self.device)
+        _chk(fn(self.h, kx_cut, kz_cut, db.data_ptr(), out.data_ptr(), scratch.data_ptr(), n), name)
+        self._post_keep = scratch
+        return out
+
+    def post_pressure(self, kx_cut, kz_cut, db):
+        return self._post(self.lib.chan_post_pressure, "chan_post_pressure", kx_cut, kz_cut, db)
+
+    def post_strain_norm(self, kx_cut, kz_cut, db):
+        return self._post(self.lib.chan_post_strain_norm, "chan_post_strain_norm", kx_cut, kz_cut, db)
+
+    def post_sgs(self, kx_cut, kz_cut, db):
+        return self._post(self.lib.chan_post_sgs, "chan_post_sgs", kx_cut, kz_cut, db, lead=(6,))
 
     def stats(self, flags):
         out = np.zeros((10, self.ny))

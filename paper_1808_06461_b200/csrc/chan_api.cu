@@ -13,6 +13,7 @@
 #include "chan_fft.cuh"
 #include "chan_planekernels.cuh"
 #include "chan_plan.h"
+#include "chan_post.cuh"
 #include "chan_ykernels.cuh"
 #include "chan_ysweeps.cuh"
 
@@ -803,6 +804,74 @@ int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts) 
             host_ms[h->prof_cls[i]] += ms; host_counts[h->prof_cls[i]] += 1;
         }
     }
+    return CHAN_OK;
+}
+
+// ---- post-processing of a stored database (NEXT-2) -----------------------------------------------------
+size_t chan_post_scratch_bytes(const chan_t* h, int kxc, int kzc) {
+    if (!h || kxc < 0 || kzc < 0 || kxc > h->P.nxh - 1 || kzc > h->P.nzh - 1) return 0;
+    return (size_t)7 * h->P.ny * (2 * kzc + 1) * (kxc + 1) * 16;
+}
+
+static int post_check(chan_t* h, int kxc, int kzc, const void* db, const void* out, const void* scratch, size_t sbytes, PostParams& Q) {
+    if (!h || !db || !out || !scratch) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
+    if (sbytes < chan_post_scratch_bytes(h, kxc, kzc)) return CHAN_ENOSPACE;
+    Q.ny = P.ny; Q.nr = 2 * kzc + 1; Q.npk = kxc + 1; Q.kzc = kzc; Q.nz = P.nz;
+    Q.B1 = h->tab[0][0]; Q.A2 = h->tab[0][1]; Q.B2 = h->tab[0][2]; Q.lu1 = h->tab[0][3];
+    Q.kx = h->kx; Q.kz = h->kz; Q.wm = h->wm; Q.wp = h->wp; Q.nu = P.nu;
+    return CHAN_OK;
+}
+
+int chan_post_pressure(chan_t* h, int kxc, int kzc, const void* dev_db, void* dev_p, void* dev_scratch, size_t scratch_bytes) {
+    PostParams Q;
+    int rc = post_check(h, kxc, kzc, dev_db, dev_p, dev_scratch, scratch_bytes, Q);
+    if (rc) return rc;
+    const size_t per = (size_t)Q.ny * Q.nr * Q.npk;
+    double2* S = (double2*)dev_scratch;
+    const unsigned g = (unsigned)((Q.nr * Q.npk + 127) / 128);
+    PB(CHAN_KC_POST); k_post_divdiv<<<g, 128, 0, h->stream>>>(Q, (const double2*)dev_db, S + per, S, 0); LAUNCHED();
+    PB(CHAN_KC_POST); k_post_pressure<<<g, 128, 0, h->stream>>>(Q, (const double2*)dev_db, S, S + per, S + 2 * per, S + 3 * per, S + 4 * per, (double2*)dev_p); LAUNCHED();
+    return CHAN_OK;
+}
+
+int chan_post_strain_norm(chan_t* h, int kxc, int kzc, const void* dev_db, void* dev_out, void* dev_scratch, size_t scratch_bytes) {
+    PostParams Q;
+    int rc = post_check(h, kxc, kzc, dev_db, dev_out, dev_scratch, scratch_bytes, Q);
+    if (rc) return rc;
+    const unsigned g = (unsigned)((Q.nr * Q.npk + 127) / 128);
+    PB(CHAN_KC_POST); k_post_divdiv<<<g, 128, 0, h->stream>>>(Q, (const double2*)dev_db, (double2*)dev_scratch, (double2*)dev_out, 1); LAUNCHED();
+    return CHAN_OK;
+}
+
+int chan_post_sgs(chan_t* h, int kxc, int kzc, const void* dev_db, void* dev_tau, void* dev_scratch, size_t scratch_bytes) {
+    PostParams Q;
+    int rc = post_check(h, kxc, kzc, dev_db, dev_tau, dev_scratch, scratch_bytes, Q);
+    if (rc) return rc;
+    if (h->isub != 0) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    const size_t per = (size_t)Q.ny * Q.nr * Q.npk;
+    // the stored velocities into the handle's own u, v, w (zeros beyond the cutoff; the vorticity slots are cleared: the
+    // seventh product of the filter pass is not used), then the library's dealiased product path, pruned to the cutoff
+    for (double2* f : {h->u, h->s1, h->w, h->ox, h->oz}) CK(cudaMemsetAsync(f, 0, h->F, h->stream));
+    double2* keep_omy = h->omy;               // om_y is state: read a zero field instead of clobbering it
+    PB(CHAN_KC_POST); k_post_scatter<<<296, 256, 0, h->stream>>>(Q, P.nxh, (const double2*)dev_db, h->u, h->s1, h->w); LAUNCHED();
+    // v is state as well: the scattered v lives in the scratch field s1 for the duration of the pass
+    double2* keep_v = h->v;
+    h->v = h->s1; h->omy = h->ox;
+    FieldPtrsW o;
+    double2* T = (double2*)dev_scratch;
+    for (int k = 0; k < 7; ++k) o.f[k] = T + (size_t)k * per;
+    const int f32 = h->out_f32;
+    h->out_f32 = 0;
+    rc = run_planes(h, 7, o, kxc, kzc);
+    h->out_f32 = f32; h->v = keep_v; h->omy = keep_omy;
+    if (rc) return rc;
+    PB(CHAN_KC_POST); k_post_sub<<<296, 256, 0, h->stream>>>(6 * per, (const double2*)dev_db + 3 * per, T, (double2*)dev_tau); LAUNCHED();
+    // u, w, om_x, om_z were clobbered: rebuild them from the state if there is one
+    if (h->have_state) return run_derive(h);
     return CHAN_OK;
 }
 
