@@ -126,6 +126,27 @@ typedef struct {
 } chan_run_t;
 int chan_run(chan_t* h, const chan_run_t* r, long long* snapshots);
 
+/* ---- mesh tools of the paper's section 2.3 (NEXT-4; Fig. 2.3); HOST only, no handle, no device ----------
+ * "The most numerically sensitive operation ... is the solution of the bilaplacian operator, which requires the solution
+ * of multiple homogeneous Helmholtz equations ... very thin boundary layers near the wall" (L100).
+ * chan_mesh_helmholtz_error: the paper's test.  For the compact second-derivative rows of reading R4 on the mesh
+ * host_y[ny] it solves phi'' = lambda phi with phi = 1 at one wall and 0 at the other and returns, for each wall, the
+ * maximum over the first nfirst interior points of |phi_j - phi_exact(y_j)|: host_err2[0] for y = -1, [1] for y = +1.
+ * lambda is the caller's worst case, k_max^2 + 1/(beta_3 nu dt) (beta_3 = 1/6).
+ * chan_mesh_optimize: the paper's remedy (L102: "slightly displacing the first 20 grid points in order to minimize the
+ * error of the most dangerous solutions without affecting too much the individual grid spacing").  Points 1..npoints
+ * from each wall are moved, each by at most max_shift (< 1/2) times the smaller of its two original neighbouring
+ * spacings, by a deterministic cyclic coordinate search (`sweeps` rounds with a halving step) that minimises the error
+ * above over the first npoints + 3 points; a displacement is only accepted if the mesh stays admissible for the
+ * unpivoted solves (every elimination pivot of B2 - sigma A2 negative for sigma = 0, lambda/100, lambda: without this
+ * guard the search walks into meshes whose second-derivative operator has eigenvalues in the right half plane -- the
+ * instability L102 mentions).  The paper prints neither its objective nor its optimiser: this is reading R23 of
+ * DESIGN.md.  host_y is updated in place; the errors before and after (two walls each) are optional outputs.
+ * CHAN_EINVAL: bad sizes, non-monotone or inadmissible input mesh, max_shift outside (0, 1/2). */
+int chan_mesh_helmholtz_error(int ny, const double* host_y, double lambda, int nfirst, double* host_err2);
+int chan_mesh_optimize(int ny, double* host_y, int npoints, double lambda, double max_shift, int sweeps, double* host_err_before2,
+                       double* host_err_after2);
+
 /* ---- post-processing of a stored database (NEXT-2; section 3.2) ---------------------------
  * dev_db is a complex128 database as written by chan_filter_store / chan_step_filter / chan_run with the same
  * cutoffs, [10][ny][2 kz_cut+1][kx_cut+1].  The handle supplies the mesh, its compact operators, nu and the box; it

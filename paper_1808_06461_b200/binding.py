@@ -26,6 +26,7 @@ EXPORTS = [
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
     "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe", "chan_debug_fma_peak", "chan_set_filter_precision", "chan_run",
     "chan_post_scratch_bytes", "chan_post_pressure", "chan_post_strain_norm", "chan_post_sgs",
+    "chan_mesh_helmholtz_error", "chan_mesh_optimize",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
                   "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged", "post"]
@@ -106,6 +107,8 @@ def load():
         "chan_debug_fma_peak": (i, [vp, C.POINTER(C.c_double)]),
         "chan_set_filter_precision": (i, [vp, i]),
         "chan_run": (i, [vp, C.POINTER(Run), C.POINTER(C.c_longlong)]),
+        "chan_mesh_helmholtz_error": (i, [i, vp, d, i, vp]),
+        "chan_mesh_optimize": (i, [i, vp, i, d, d, i, vp, vp]),
         "chan_post_scratch_bytes": (sz, [vp, i, i]),
         "chan_post_pressure": (i, [vp, i, i, vp, vp, vp, sz]),
         "chan_post_strain_norm": (i, [vp, i, i, vp, vp, vp, sz]),
@@ -121,6 +124,23 @@ def load():
 def _chk(status, where):
     if status != OK:
         raise ChanError(status, where)
+
+
+def mesh_helmholtz_error(y, lam, nfirst):
+    """chan_mesh_helmholtz_error: (error at y = -1, error at y = +1)."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    out = np.zeros(2)
+    _chk(load().chan_mesh_helmholtz_error(y.size, y.ctypes.data, float(lam), int(nfirst), out.ctypes.data), "chan_mesh_helmholtz_error")
+    return out
+
+
+def mesh_optimize(y, npoints, lam, max_shift=0.25, sweeps=8):
+    """chan_mesh_optimize: (new mesh, errors before [2], errors after [2])."""
+    y = np.array(y, dtype=np.float64, copy=True)
+    eb, ea = np.zeros(2), np.zeros(2)
+    _chk(load().chan_mesh_optimize(y.size, y.ctypes.data, int(npoints), float(lam), float(max_shift), int(sweeps), eb.ctypes.data,
+                                   ea.ctypes.data), "chan_mesh_optimize")
+    return y, eb, ea
 
 
 class Channel:

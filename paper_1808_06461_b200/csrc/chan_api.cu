@@ -807,6 +807,15 @@ int chan_debug_profile_read(chan_t* h, double* host_ms, long long* host_counts) 
     return CHAN_OK;
 }
 
+// ---- mesh tools of the paper's section 2.3 (NEXT-4), host only ------------------------------------------------------
+int chan_mesh_helmholtz_error(int ny, const double* host_y, double lambda, int nfirst, double* host_err2) {
+    return mesh_helmholtz_error(ny, host_y, lambda, nfirst, host_err2);
+}
+int chan_mesh_optimize(int ny, double* host_y, int npoints, double lambda, double max_shift, int sweeps, double* host_err_before2,
+                       double* host_err_after2) {
+    return mesh_optimize(ny, host_y, npoints, lambda, max_shift, sweeps, host_err_before2, host_err_after2);
+}
+
 // ---- post-processing of a stored database (NEXT-2) -----------------------------------------------------
 size_t chan_post_scratch_bytes(const chan_t* h, int kxc, int kzc) {
     if (!h || kxc < 0 || kzc < 0 || kxc > h->P.nxh - 1 || kzc > h->P.nzh - 1) return 0;

@@ -235,6 +235,126 @@ bool make_fft_plan(int n, int fused_last, int maxr, FftPlan& F) {
 
 }  // namespace
 
+// ---- section 2.3 of the paper (L100-102): wall-layer error of the homogeneous Helmholtz solutions and the mesh remedy ----
+namespace {
+
+// D2 rows (A2, B2) of the mesh y for rows j in [lo, hi] into the [ny][7] tables (rows 0 and ny-1 are not used)
+bool d2_rows(const std::vector<double>& y, int lo, int hi, std::vector<double>& A2, std::vector<double>& B2) {
+    const int ny = (int)y.size();
+    for (int j = std::max(lo, 1); j <= std::min(hi, ny - 2); ++j) {
+        const int room = std::min(j, ny - 1 - j), s = std::min(3, room);
+        std::vector<int> off;
+        for (int m = -s; m <= s; ++m) off.push_back(m);
+        if (!compact_row(y, j, off, off, 2, &A2[(size_t)j * 7], &B2[(size_t)j * 7])) return false;
+    }
+    return true;
+}
+
+// max over the first `nfirst` interior points next to the wall `side` (0: y = -1, 1: y = +1) of |phi_j - phi(y_j)|, phi the
+// solution of phi'' = lam phi with phi = 1 at that wall and 0 at the other one
+bool wall_error(const std::vector<double>& y, const std::vector<double>& A2, const std::vector<double>& B2, double lam, int nfirst,
+                int side, double* err) {
+    const int ny = (int)y.size();
+    std::vector<ld> T((size_t)ny * 7, 0.0L), x(ny, 0.0L);
+    for (int j = 1; j + 1 < ny; ++j)
+        for (int k = 0; k < 7; ++k) T[(size_t)j * 7 + k] = (ld)B2[(size_t)j * 7 + k] - (ld)lam * (ld)A2[(size_t)j * 7 + k];
+    T[3] = 1.0L; T[(size_t)(ny - 1) * 7 + 3] = 1.0L;
+    x[side == 0 ? 0 : ny - 1] = 1.0L;
+    if (!band_solve(ny, T, x)) return false;
+    const ld k = sqrtl((ld)lam);
+    ld e = 0;
+    for (int n = 1; n <= nfirst && n + 1 < ny; ++n) {
+        const int j = side == 0 ? n : ny - 1 - n;
+        const ld d = side == 0 ? 1.0L + (ld)y[j] : 1.0L - (ld)y[j];      // distance from the wall that carries the 1
+        const ld ex = expl(-k * d) * (1.0L - expl(-2.0L * k * (2.0L - d))) / (1.0L - expl(-4.0L * k));
+        e = std::max(e, fabsl(x[j] - ex));
+    }
+    *err = (double)e;
+    return true;
+}
+
+// Admissibility guard of the optimiser: every pivot of the unpivoted elimination of B2 - sigma A2 (Dirichlet rows) is
+// negative, for sigma = 0, lam/100 and lam.  On admissible meshes (real negative D2-Dirichlet spectrum) all
+// pivots are negative for every sigma >= 0; a displaced mesh whose spectrum has crossed to the right half plane shows
+// positive pivots already at sigma = 0, and the marching kernels, which eliminate without pivoting, need the former.
+bool pivots_negative(const std::vector<double>& A2, const std::vector<double>& B2, int ny, double lam) {
+    const double sig[3] = {0.0, lam * 0.01, lam};
+    for (double sg : sig) {
+        std::vector<ld> W((size_t)ny * 7, 0.0L);
+        for (int j = 1; j + 1 < ny; ++j)
+            for (int k = 0; k < 7; ++k) W[(size_t)j * 7 + k] = (ld)B2[(size_t)j * 7 + k] - (ld)sg * (ld)A2[(size_t)j * 7 + k];
+        W[3] = -1.0L; W[(size_t)(ny - 1) * 7 + 3] = -1.0L;
+        for (int j = 0; j < ny; ++j) {
+            const ld piv = W[(size_t)j * 7 + 3];
+            if (!(piv < 0.0L)) return false;
+            for (int t = 1; t <= 3 && j + t < ny; ++t) {
+                const ld l = W[(size_t)(j + t) * 7 + 3 - t] / piv;
+                for (int cc = 1; cc <= 3; ++cc) W[(size_t)(j + t) * 7 + 3 - t + cc] -= l * W[(size_t)j * 7 + 3 + cc];
+            }
+        }
+    }
+    return true;
+}
+
+}  // namespace
+
+int mesh_helmholtz_error(int ny, const double* y, double lam, int nfirst, double* err2) {
+    if (ny < 8 || !y || !(lam > 0) || nfirst < 1 || !err2) return CHAN_EINVAL;
+    std::vector<double> yy(y, y + ny), A2((size_t)ny * 7, 0.0), B2((size_t)ny * 7, 0.0);
+    for (int j = 1; j < ny; ++j) if (!(yy[j] > yy[j - 1])) return CHAN_EINVAL;
+    if (!d2_rows(yy, 1, ny - 2, A2, B2)) return CHAN_EINVAL;
+    for (int side = 0; side < 2; ++side) if (!wall_error(yy, A2, B2, lam, nfirst, side, &err2[side])) return CHAN_EINVAL;
+    return CHAN_OK;
+}
+
+// Cyclic coordinate search with a halving step: point j (1 <= j <= npoints from each wall) may move by at most
+// max_shift times the smaller of its two ORIGINAL neighbouring spacings, which keeps the mesh monotone for max_shift < 1/2
+// and bounds the change of every spacing by 2 max_shift of the original one.  Objective: the wall error above at the
+// wall the point belongs to.  Deterministic; the two walls are treated independently.
+int mesh_optimize(int ny, double* y, int npoints, double lam, double max_shift, int sweeps, double* err_before, double* err_after) {
+    if (ny < 16 || !y || npoints < 1 || 2 * (npoints + 4) > ny || !(lam > 0) || !(max_shift > 0) || max_shift >= 0.5 || sweeps < 1) return CHAN_EINVAL;
+    std::vector<double> y0(y, y + ny), yy(y0), A2((size_t)ny * 7, 0.0), B2((size_t)ny * 7, 0.0);
+    for (int j = 1; j < ny; ++j) if (!(yy[j] > yy[j - 1])) return CHAN_EINVAL;
+    if (!d2_rows(yy, 1, ny - 2, A2, B2)) return CHAN_EINVAL;
+    if (!pivots_negative(A2, B2, ny, lam)) return CHAN_EINVAL;      // the mesh handed in is not admissible itself
+    const int nfirst = npoints + 3;
+    // a mesh that is symmetric about y = 0 stays so: the mirror point moves with its twin and one wall is optimised
+    bool sym = true;
+    for (int j = 0; j < ny; ++j) if (y0[j] != -y0[ny - 1 - j]) sym = false;
+    for (int side = 0; side < (sym ? 1 : 2); ++side) {
+        double best;
+        if (!wall_error(yy, A2, B2, lam, nfirst, side, &best)) return CHAN_EINVAL;
+        if (err_before) { err_before[side] = best; if (sym) err_before[1] = best; }
+        double step = max_shift;
+        auto place = [&](int j, double v) {
+            yy[j] = v;
+            bool ok = d2_rows(yy, j - 3, j + 3, A2, B2);
+            if (sym) { const int jm = ny - 1 - j; yy[jm] = -v; ok = ok && d2_rows(yy, jm - 3, jm + 3, A2, B2); }
+            return ok;
+        };
+        for (int sw = 0; sw < sweeps; ++sw, step *= 0.5) {
+            for (int n = 1; n <= npoints; ++n) {
+                const int j = side == 0 ? n : ny - 1 - n;
+                const double h = std::min(y0[j] - y0[j - 1], y0[j + 1] - y0[j]);
+                const double keep = yy[j];
+                double arg = keep;
+                for (int sg = -1; sg <= 1; sg += 2) {
+                    double cand = keep + sg * step * h;
+                    cand = std::min(std::max(cand, y0[j] - max_shift * h), y0[j] + max_shift * h);
+                    if (cand == keep) continue;
+                    double e;
+                    if (!place(j, cand) || !wall_error(yy, A2, B2, lam, nfirst, side, &e)) return CHAN_EINVAL;
+                    if (e < best && pivots_negative(A2, B2, ny, lam)) { best = e; arg = cand; }
+                }
+                if (!place(j, arg)) return CHAN_EINVAL;
+            }
+        }
+        if (err_after) { err_after[side] = best; if (sym) err_after[1] = best; }
+    }
+    for (int j = 0; j < ny; ++j) y[j] = yy[j];
+    return CHAN_OK;
+}
+
 // Stage lists of the two transform lengths.  xfuse: 4 | 8 = radix of the x stage fused with the products (0: the one
 // that gives the shorter stage list, then the one without radix-12 stages, then 4: lighter fused stage);
 // maxr: largest radix of a z stage (0: 12); maxrx: largest radix of an x stage (0: 18 -- two shared-memory stages in

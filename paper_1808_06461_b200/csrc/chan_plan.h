@@ -45,6 +45,12 @@ struct Plan {
 // zeros, chan_debug_set_tuning() again with the caller's overrides.  Returns 0 or CHAN_EINVAL.
 int plan_ffts(Plan& P, int xfuse, int maxradix_z, int maxradix_x);
 
+// PAPER.md section 2.3 (L100-102), host only: wall-layer error of the discrete homogeneous Helmholtz solution at both walls
+// (err2[0]: y = -1, err2[1]: y = +1), and the paper's remedy (the first `npoints` mesh points of each wall displaced to
+// minimise it).  chan_plan.cpp.
+int mesh_helmholtz_error(int ny, const double* y, double lam, int nfirst, double* err2);
+int mesh_optimize(int ny, double* y, int npoints, double lam, double max_shift, int sweeps, double* err_before, double* err_after);
+
 // Returns 0 or a CHAN_E* status.
 int build_plan(Plan& P, int nx, int ny, int nz, double lx, double lz, const double* y, double re_tau, double dt,
                int half_lhs, int half_rhs, int forcing);
