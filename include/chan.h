@@ -202,7 +202,10 @@ typedef struct {
     int plane_overlap;    /* 1 (default): K2, K3, K4 as separate launches; 2: merged launches (K2 of chunk t, K3 of chunk t-1,
                              K4 of chunk t-2 interleaved in one grid; CHAN_EINVAL if not compiled for this plan; results equal
                              to rounding, not bit for bit: another kernel, another FMA contraction); get: the mode in effect */
-    int reserved[7];      /* must be 0                                                                             */
+    int z_cluster;        /* 1 (default): one CTA per z tile; 2: the tile split by rows over a 2-CTA cluster with twice the
+                             columns, half of one stage's data exchanged through distributed shared memory (CHAN_EINVAL if
+                             not compiled for this plan; measured slower on config 3-5, kept as an experiment)            */
+    int reserved[6];      /* must be 0                                                                             */
 } chan_tuning_t;
 int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t);
 int chan_debug_get_tuning(const chan_t* h, chan_tuning_t* out);

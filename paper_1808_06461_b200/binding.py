@@ -48,7 +48,7 @@ class Tuning(C.Structure):
     """chan_tuning_t of include/chan.h (0 = the plan's own choice)."""
     _fields_ = [("xfuse", C.c_int), ("maxradix_z", C.c_int), ("maxradix_x", C.c_int), ("tz", C.c_int), ("zthreads", C.c_int),
                 ("xthreads", C.c_int), ("chunk_mb", C.c_int), ("planes_per_chunk", C.c_int), ("plane_overlap", C.c_int),
-                ("reserved", C.c_int * 7)]
+                ("z_cluster", C.c_int), ("reserved", C.c_int * 6)]
 
 
 class Run(C.Structure):

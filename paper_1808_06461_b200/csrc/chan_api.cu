@@ -47,6 +47,11 @@ struct chan {
     void (*kzfwd)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int) = nullptr;
     void (*kx3)(PlaneParams, const double2*, int, double2*, int) = nullptr;
     void (*kx7)(PlaneParams, const double2*, int, double2*, int) = nullptr;
+    // 2-CTA cluster variants of the z passes (tile split by rows, twice the columns per tile), if compiled for this plan
+    void (*kzinv_c)(PlaneParams, FieldPtrs, int, int, double2*, int) = nullptr;
+    void (*kzfwd_c)(PlaneParams, const double2*, int, int, int, FieldPtrsW, double, int, int, int, int) = nullptr;
+    bool zcluster = false;     // the z passes run through them, with Tzc columns per tile
+    int Tzc = 0;
     void (*kmerged)(PlaneParams, MergedArgs) = nullptr;   // K2 | K3 | K4 of neighbouring chunks in one launch, if compiled for this plan
     bool merged = false;   // the substep's plane phase runs through kmerged
     bool zspecial = false, xspecial = false;
@@ -87,6 +92,11 @@ void choose_tiling(chan_t* h) {
     while (T > 1 && T > P.nxh) T >>= 1;
     h->Tz = U.tz ? U.tz : T;
     h->zthreads = U.zthreads ? U.zthreads : 256;
+    // row pieces narrower than 128 B (fewer than 8 columns per tile) cost ~14% per halving (config 3); the cluster variant
+    // splits the tile by rows over two CTAs and doubles the columns
+    h->Tzc = 2 * h->Tz;
+    const bool can = h->kzinv_c && h->Tzc <= 16 && h->Tzc <= P.nxh && !h->merged && (size_t)P.mz * h->Tzc * 8 <= 112 * 1024;
+    h->zcluster = can && U.z_cluster == 2;    // measured slower than one CTA per narrower tile: opt-in
     h->xthreads = U.xthreads ? U.xthreads : (((size_t)3 * P.mx * 16 > 72 * 1024) ? 256 : 128);   // <= 3 CTAs per SM: use wider CTAs
     const size_t per_plane = (size_t)(h->merged ? 19 : 13) * P.mz * P.nxh * 16;
     // zpad + xh: about 11 planes of config 5 per chunk (longer grids, smaller tails)
@@ -193,6 +203,7 @@ int run_derive(chan_t* h) {
 #define CHAN_ZPLANS(X) X(6, 1, 1, 1) X(12, 1, 1, 1) X(6, 4, 1, 1) X(6, 8, 1, 1) X(12, 6, 1, 1) X(12, 8, 1, 1) X(12, 12, 1, 1) \
     X(6, 8, 4, 1) X(6, 6, 8, 1) X(6, 8, 8, 1) X(12, 6, 8, 1) X(12, 8, 8, 1) X(12, 12, 6, 1) X(12, 12, 8, 1) X(12, 12, 12, 1) \
     X(6, 8, 8, 4) X(6, 6, 8, 8) X(6, 8, 8, 8)
+#define CHAN_ZPLANS_C(X) X(12, 12, 12, 1) X(6, 8, 8, 4) X(12, 12, 6, 1) X(12, 6, 1, 1) X(6, 8, 1, 1)
 #define CHAN_XPLANS(X) X(4, 6, 1, 1) X(4, 12, 1, 1) X(4, 6, 4, 1) X(4, 6, 6, 1) X(4, 6, 8, 1) X(4, 12, 8, 1) X(4, 6, 6, 4) X(4, 6, 6, 6) \
     X(4, 6, 8, 4) X(4, 6, 6, 8) X(4, 6, 8, 8) X(4, 12, 6, 6) X(4, 12, 6, 8) X(4, 12, 8, 8) X(8, 6, 1, 1) X(8, 12, 1, 1) X(8, 12, 6, 1) \
     X(8, 12, 12, 1) X(8, 6, 8, 1) X(8, 12, 16, 1) X(8, 18, 16, 1) X(8, 18, 1, 1) X(8, 16, 1, 1) X(8, 12, 8, 1) X(8, 6, 6, 1) X(8, 6, 6, 8) X(8, 6, 8, 4) X(8, 6, 8, 8) X(8, 12, 6, 8)
@@ -231,6 +242,11 @@ void pick_kernels(chan_t* h) {
         CHAN_XPLANS(X)
 #undef X
     }
+    // cluster z kernels: compiled for the z lists of the benchmark shapes and of the small parity cases
+    h->kzinv_c = nullptr; h->kzfwd_c = nullptr;
+#define X(a, b, c, d) { const int r[4] = {a, b, c, d}; if (same_list(P.fz.radix, 4, r)) { h->kzinv_c = k_zfft_inv_c<a, b, c, d>; h->kzfwd_c = k_zfft_fwd_c<a, b, c, d>; } }
+    CHAN_ZPLANS_C(X)
+#undef X
     // merged plane kernel: compiled for the (z list, x list) pairs of the benchmark shapes only (each pair is one more
     // instantiation of all three bodies); any other plan runs the three kernels one after the other
     h->kmerged = nullptr;
@@ -249,6 +265,12 @@ size_t merged_smem(const chan_t* h) {
 }
 
 int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, int npl) {
+    if (h->zcluster) {
+        const int T = h->Tzc;
+        dim3 g(2 * ((Q.nxh + T - 1) / T), npl, nf);
+        PB(CHAN_KC_ZFFT_INV); h->kzinv_c<<<g, 256, (size_t)Q.mz * T * 8, h->stream>>>(Q, in, j0, npl, h->zpad, T); LAUNCHED();
+        return CHAN_OK;
+    }
     const int T = h->Tz;
     const size_t sm = (size_t)Q.mz * T * 16;
     dim3 g((Q.nxh + T - 1) / T, npl, nf);
@@ -256,6 +278,13 @@ int zinv(chan_t* h, const PlaneParams& Q, const FieldPtrs& in, int nf, int j0, i
     return CHAN_OK;
 }
 int zfwd(chan_t* h, const PlaneParams& Q, int pin, int nf, int j0, int npl, const FieldPtrsW& out, double scale, int filt, int kxc, int kzc) {
+    if (h->zcluster) {
+        const int T = h->Tzc;
+        dim3 g(2 * ((pin + T - 1) / T), npl, nf);
+        PB(filt ? CHAN_KC_ZFFT_FWD_FILTER : CHAN_KC_ZFFT_FWD);
+        h->kzfwd_c<<<g, 256, (size_t)Q.mz * T * 8, h->stream>>>(Q, h->xh, pin, j0, npl, out, scale, filt, kxc, kzc, T); LAUNCHED();
+        return CHAN_OK;
+    }
     const int T = h->Tz;
     const size_t sm = (size_t)Q.mz * T * 16;
     dim3 g((pin + T - 1) / T, npl, nf);
@@ -392,6 +421,7 @@ int configure(chan_t* h) {
     if (h->tune.plane_overlap == 2 && !h->kmerged) return CHAN_EINVAL;
     h->merged = h->kmerged && h->tune.plane_overlap == 2;   // measured on config 5: no gain over separate launches, so opt-in
     choose_tiling(h);
+    if (h->tune.z_cluster == 2 && !h->zcluster) return CHAN_EINVAL;
     if ((size_t)4 * h->P.mx * 16 > 220 * 1024 || (size_t)h->P.mz * h->Tz * 16 > 220 * 1024) return CHAN_EINVAL;
     if ((size_t)15 * h->P.ny * 8 > 220 * 1024) return CHAN_EINVAL;   // mean-mode solve lives in shared memory
     h->need = carve(h, nullptr);
@@ -442,7 +472,7 @@ int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t) {
     if ((t->xfuse && t->xfuse != 4 && t->xfuse != 8) || (t->maxradix_z && (t->maxradix_z < 2 || t->maxradix_z > 12)) ||
         (t->maxradix_x && (t->maxradix_x < 2 || t->maxradix_x > 18)) || (t->tz && !pow2(t->tz)) ||
         (t->zthreads && (t->zthreads < 32 || t->zthreads > 256)) || (t->xthreads && (t->xthreads < 32 || t->xthreads > 256)) ||
-        t->chunk_mb < 0 || t->plane_overlap < 0 || t->plane_overlap > 2)
+        t->chunk_mb < 0 || t->plane_overlap < 0 || t->plane_overlap > 2 || t->z_cluster < 0 || t->z_cluster > 2)
         return CHAN_EINVAL;
     const chan_tuning_t old = h->tune;
     const FftPlan ofx = h->P.fx, ofz = h->P.fz;
@@ -463,6 +493,8 @@ int chan_debug_get_tuning(const chan_t* h, chan_tuning_t* out) {
     out->chunk_mb = h->tune.chunk_mb ? h->tune.chunk_mb : 3072;
     out->planes_per_chunk = h->pc;
     out->plane_overlap = h->merged ? 2 : 1;
+    out->z_cluster = h->zcluster ? 2 : 1;
+    if (h->zcluster) out->tz = h->Tzc;
     return CHAN_OK;
 }
 
@@ -500,6 +532,10 @@ int chan_bind(chan_t* h, void* dev_workspace, size_t bytes, void* cuda_stream) {
     CK(cudaFuncSetAttribute((const void*)h->kx3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)3 * P.mx * 16)));
     CK(cudaFuncSetAttribute((const void*)h->kx7, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)4 * P.mx * 16)));
     CK(cudaFuncSetAttribute(k_mean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)15 * P.ny * 8)));
+    if (h->zcluster) {
+        CK(cudaFuncSetAttribute((const void*)h->kzinv_c, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P.mz * h->Tzc * 8)));
+        CK(cudaFuncSetAttribute((const void*)h->kzfwd_c, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P.mz * h->Tzc * 8)));
+    }
     if (h->merged) CK(cudaFuncSetAttribute((const void*)h->kmerged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)merged_smem(h)));
     h->bound = true; h->have_state = false; h->isub = 0; h->nsamples = 0;
     return CHAN_OK;
@@ -774,7 +810,8 @@ int chan_debug_describe(const chan_t* h, char* buf, size_t n) {
     for (size_t k = 0; k < rz.size(); ++k) s += (k ? "," : " ") + std::to_string(rz[k]);
     s += "  specialised x/z: " + std::to_string((int)h->xspecial) + "/" + std::to_string((int)h->zspecial);
     s += "  merged plane launches: " + std::to_string((int)h->merged);
-    s += "  tz " + std::to_string(h->Tz) + "  threads x/z " + std::to_string(h->xthreads) + "/" + std::to_string(h->zthreads);
+    s += "  z cluster: " + std::to_string((int)h->zcluster);
+    s += "  tz " + std::to_string(h->zcluster ? h->Tzc : h->Tz) + "  threads x/z " + std::to_string(h->xthreads) + "/" + std::to_string(h->zthreads);
     s += "  planes per chunk " + std::to_string(h->pc);
     std::strncpy(buf, s.c_str(), n - 1);
     buf[n - 1] = 0;

@@ -242,13 +242,14 @@ struct FieldPtrsW { double2* f[8]; };
 // =====================================================================================================
 // M > 0: the sub-block length as a compile-time constant (specialised kernels), M = 0: taken from the stage.
 template <int R, bool INV, bool DIT, int M = 0, class Src, class Dst>
-CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int T, int tid, int nt) {
-    const int m = M > 0 ? M : S.m, ncur = R * m, nb = n / R;
+CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int T, int tid, int nt, int half = -1) {
+    // half >= 0: only that half of the butterflies (the cluster kernels split a stage between two CTAs)
+    const int m = M > 0 ? M : S.m, ncur = R * m, nb = half < 0 ? n / R : n / R / 2, b0 = half > 0 ? nb : 0;
     const int total = nb * T;
     int lgT = 0;
     while ((1 << lgT) < T) ++lgT;               // T is a power of two
     for (int w = tid; w < total; w += nt) {
-        const int b = w >> lgT, t = w & (T - 1);
+        const int b = b0 + (w >> lgT), t = w & (T - 1);
         const int blk = b / m, p = b - blk * m;
         c2 tw[R - 1 > 0 ? R - 1 : 1];
         if (m > 1) load_twiddles<R>(S, m, p, tw);
@@ -463,6 +464,107 @@ template <int R0, int R1, int R2, int R3>
 __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
     extern __shared__ double2 smem_raw[];
     zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, filt, kxc, kzc, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+}
+#endif
+
+// ---- 2-CTA cluster variants of the z passes ------------------------------------------------------------------------
+// Where a tile of 8 columns (128-byte row pieces) does not fit the shared memory that lets two CTAs share an SM
+// (config 5: 1728 rows x 8 columns x 16 B = 221 KB), the tile is split BY ROWS between the two CTAs of a thread-block
+// cluster: rank r keeps rows [r n/2, (r+1) n/2).  Only the stage with the longest stride (R0, sub-block M0 = n/R0) couples
+// the halves: its butterfly p + k M0, k < R0, has R0/2 elements in each half (R0 even), so that stage is split by
+// butterflies and half of its shared-memory traffic goes through distributed shared memory; every other stage works on
+// blocks of M0 rows that lie inside one half.  Inverse (DIF): the coupling stage is the first one (reads global memory,
+// writes both halves), then a cluster barrier.  Forward (DIT): it is the last one (reads both halves, writes global
+// memory), between two cluster barriers (the partner's shared memory must outlive the reads).
+struct ZInvIOc {
+    ZInvIO b; c2* smr; int eoff, nh;            // partner's half, first row of this half, rows per half
+    CHAN_HD c2 load(int e, int t) const { return b.gin ? b.load(e, t) : b.sm[(e - eoff) * b.T + t]; }
+    CHAN_HD void store(int e, int t, c2 v) const {
+        if (b.gout) { b.store(e, t, v); return; }
+        const int el = e - eoff;
+        if ((unsigned)el < (unsigned)nh) b.sm[el * b.T + t] = v; else smr[(el < 0 ? el + nh : el - nh) * b.T + t] = v;
+    }
+};
+struct ZFwdIOc {
+    ZFwdIO b; const c2* smr; int eoff, nh;
+    CHAN_HD c2 load(int e, int t) const {
+        if (b.gin) return b.load(e, t);
+        const int el = e - eoff;
+        return ((unsigned)el < (unsigned)nh) ? b.sm[el * b.T + t] : smr[(el < 0 ? el + nh : el - nh) * b.T + t];
+    }
+    CHAN_HD void store(int e, int t, c2 v) const { if (b.gout) b.store(e, t, v); else b.sm[(e - eoff) * b.T + t] = v; }
+};
+
+#ifdef __CUDACC__
+}  // namespace chn
+#include <cooperative_groups.h>
+namespace chn {
+template <int R0, int R1, int R2, int R3>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(256, 2) k_zfft_inv_c(CHAN_ZARGS_INV) {
+    extern __shared__ double2 smem_raw[];
+    namespace cg = cooperative_groups;
+    constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
+    static_assert(NS >= 2 && R0 % 2 == 0 && (R1 * R2 * R3) % 2 == 0, "the cluster split needs an even first radix, an even sub-block and a second stage");
+    cg::cluster_group cl = cg::this_cluster();
+    const int rank = (int)cl.block_rank();
+    const int p0 = (int)(blockIdx.x >> 1) * T, jc = blockIdx.y, fi = blockIdx.z;
+    constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
+    ZInvIOc io;
+    io.b = make_zinv_io(P, T, reinterpret_cast<c2*>(smem_raw), in.f[fi] + (size_t)(j0 + jc) * P.nm,
+                        zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
+    io.smr = reinterpret_cast<c2*>(cl.map_shared_rank(smem_raw, rank ^ 1));
+    io.nh = mz / 2; io.eoff = rank * io.nh;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    io.b.gin = true; io.b.gout = false;
+    zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt, rank);
+    cl.sync();
+    io.b.gin = false; io.b.gout = (NS == 2);
+    zpass<R1, true, false, M1>(io, io, P.fz.st[1], mz, T, tid, nt, rank);
+    if constexpr (NS > 2) {
+        __syncthreads();
+        io.b.gout = (NS == 3);
+        zpass<R2, true, false, M2>(io, io, P.fz.st[2], mz, T, tid, nt, rank);
+    }
+    if constexpr (NS > 3) {
+        __syncthreads();
+        io.b.gout = true;
+        zpass<R3, true, false, 1>(io, io, P.fz.st[3], mz, T, tid, nt, rank);
+    }
+}
+template <int R0, int R1, int R2, int R3>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(256, 2) k_zfft_fwd_c(CHAN_ZARGS_FWD) {
+    extern __shared__ double2 smem_raw[];
+    namespace cg = cooperative_groups;
+    constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
+    static_assert(NS >= 2 && R0 % 2 == 0 && (R1 * R2 * R3) % 2 == 0, "the cluster split needs an even first radix, an even sub-block and a second stage");
+    cg::cluster_group cl = cg::this_cluster();
+    const int rank = (int)cl.block_rank();
+    const int p0 = (int)(blockIdx.x >> 1) * T, jc = blockIdx.y, fi = blockIdx.z;
+    const int j = j0 + jc;
+    constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
+    ZFwdIOc io;
+    io.b = make_zfwd_io(P, T, reinterpret_cast<c2*>(smem_raw), xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin,
+                        zfwd_plane(P, out.f[fi], j, filt, kxc, kzc), pin, p0, scale, filt, kxc, kzc);
+    io.smr = reinterpret_cast<const c2*>(cl.map_shared_rank(smem_raw, rank ^ 1));
+    io.nh = mz / 2; io.eoff = rank * io.nh;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    io.b.gin = true; io.b.gout = false;
+    if constexpr (NS > 3) {
+        zpass<R3, false, true, 1>(io, io, P.fz.st[3], mz, T, tid, nt, rank);
+        __syncthreads();
+        io.b.gin = false;
+    }
+    if constexpr (NS > 2) {
+        zpass<R2, false, true, M2>(io, io, P.fz.st[2], mz, T, tid, nt, rank);
+        __syncthreads();
+        io.b.gin = false;
+    }
+    zpass<R1, false, true, M1>(io, io, P.fz.st[1], mz, T, tid, nt, rank);
+    io.b.gin = false;
+    cl.sync();
+    io.b.gout = true;
+    zpass<R0, false, true, M0>(io, io, P.fz.st[0], mz, T, tid, nt, rank);
+    cl.sync();
 }
 #endif
 

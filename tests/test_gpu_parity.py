@@ -682,3 +682,24 @@ def test_postprocessing_of_the_stored_database(B):
     tau = torch.empty((6,) + tuple(db.shape[1:]), dtype=torch.complex128, device="cuda")
     assert ch.lib.chan_post_sgs(ch.h, kxc, kzc, db.data_ptr(), tau.data_ptr(), big.data_ptr(), n) == B.ESTATE    # mid-step
     ch.close()
+
+
+@pytest.mark.parametrize("name,tz", [("mid", 8), ("cfg1", 4)])
+def test_cluster_z_passes_equal_single_cta_z_passes(B, name, tz):
+    """chan_tuning_t.z_cluster: the z tile split by rows over a 2-CTA cluster (the first inverse / last forward stage
+    exchanges half of its data through distributed shared memory) against one CTA per tile: a step, the fused filter
+    (ragged last tile: the filter's 12 columns in tiles of 16 on "mid") and the nonlinear term, equal to rounding."""
+    c = inputs.config(name)
+    v, phi, omy = seeded_state(c, 20.0 if name == "cfg1" else 1.0)
+    res = []
+    for zc in (1, 2):
+        ch = B.Channel(c["nx"], c["ny"], c["nz"], c["lx"], c["lz"], c["y"], c["re"], c["dt"], tuning=dict(z_cluster=zc, tz=tz)).bind("cuda:0")
+        t = ch.debug_get_tuning()
+        assert t["z_cluster"] == zc and t["tz"] == (2 * tz if zc == 2 else tz)
+        ch.set_state(v, phi, omy, c["U"], c["W"])
+        ch.step()
+        db = ch.step_filter(*c["cut"])
+        res.append([db.clone()] + [x.clone() for x in ch.get_state()] + [ch.debug_get_field(f) for f in (B.F_H1, B.F_H2, B.F_H3)])
+        ch.close()
+    for a, b in zip(*res):
+        assert rel(a, b.cpu().numpy()) < 1e-13
