@@ -200,18 +200,22 @@ CHAN_HD void pass_item(const Src& src, const Dst& dst, int q, int base, int m, c
 #pragma unroll
     for (int k = 0; k < R; ++k) a[k] = src.load(base + k * m, q);
     if constexpr (R > 12) {
+        // w^k as three interleaved running products (k mod 3), each stepping by w^3: a single chain of R-2 dependent
+        // complex products was the largest fixed-latency stall of the x pass (ncu: "wait"), three chains a third as deep
         const c2 w1 = INV ? mk(w[0].x, -w[0].y) : w[0];
-        if (DIT && twiddled) {
-            c2 wk = w1;
+        auto twiddle_all = [&]() {
+            const c2 w2 = cmul(w1, w1), w3 = cmul(w2, w1);
+            c2 c0 = w3, c1 = w1, c2_ = w2;               // next powers with k = 0, 1, 2 (mod 3): w^3, w^1, w^2
 #pragma unroll
-            for (int k = 1; k < R; ++k) { a[k] = cmul(a[k], wk); if (k + 1 < R) wk = cmul(wk, w1); }
-        }
+            for (int k = 1; k < R; ++k) {
+                if (k % 3 == 1) { a[k] = cmul(a[k], c1); if (k + 3 < R) c1 = cmul(c1, w3); }
+                else if (k % 3 == 2) { a[k] = cmul(a[k], c2_); if (k + 3 < R) c2_ = cmul(c2_, w3); }
+                else { a[k] = cmul(a[k], c0); if (k + 3 < R) c0 = cmul(c0, w3); }
+            }
+        };
+        if (DIT && twiddled) twiddle_all();
         bfly<R, INV>(a);
-        if (!DIT && twiddled) {
-            c2 wk = w1;
-#pragma unroll
-            for (int k = 1; k < R; ++k) { a[k] = cmul(a[k], wk); if (k + 1 < R) wk = cmul(wk, w1); }
-        }
+        if (!DIT && twiddled) twiddle_all();
     } else {
         if (DIT && twiddled) {
 #pragma unroll
@@ -256,6 +260,26 @@ CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int
         pass_item<R, INV, DIT>(src, dst, t, blk * ncur + p, m, tw, m > 1);
     }
 }
+// L2 prefetch of the global inputs of every round but the first of the stage that reads global memory: a thread owns
+// ceil(nb T / nt) butterflies of that stage and only the first one's loads are in flight when it starts; the later rounds
+// then find their rows in L2 (about a third of the DRAM latency) without holding registers for them.
+#ifndef CHAN_ZPREFETCH
+#define CHAN_ZPREFETCH 1
+#endif
+template <int R, int M, class Src>
+CHAN_HD void zprefetch(const Src& src, int n, int T, int tid, int nt) {
+#if CHAN_ZPREFETCH
+    const int m = M, ncur = R * m, nb = n / R, total = nb * T;
+    int lgT = 0;
+    while ((1 << lgT) < T) ++lgT;
+    for (int w = tid + nt; w < total; w += nt) {
+        const int b = w >> lgT, t = w & (T - 1);
+        const int blk = b / m, p = b - blk * m;
+#pragma unroll
+        for (int k = 0; k < R; ++k) src.prefetch(blk * ncur + p + k * m, t);
+    }
+#endif
+}
 template <bool INV, bool DIT, class Src, class Dst>
 CHAN_HD void zpass_any(const Src& src, const Dst& dst, const FftStage& S, int n, int T, int tid, int nt) {
     switch (S.R) {
@@ -288,6 +312,13 @@ struct ZInvIO {
         if (!gout) { sm[e * T + t] = v; return; }
         if (t < tcount) ststream(dst + (size_t)e * nxh + p0 + t, v);
     }
+    CHAN_HD void prefetch(int e, int t) const {      // the global element load(e, t) will read, into L2
+#ifdef __CUDA_ARCH__
+        int s = -1;
+        if (e < nzh) s = e; else if (e > mz - nzh) s = e - (mz - nz);
+        if (s >= 0 && t < tcount) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + (size_t)s * nxh + p0 + t));
+#endif
+    }
 };
 CHAN_HD void zinv_phase(int ph, int tid, int nt, const PlaneParams& P, int T, c2* sm, const double2* src, double2* dst, int p0) {
     ZInvIO io;
@@ -311,6 +342,11 @@ struct ZFwdIO {
     CHAN_HD c2 load(int e, int t) const {
         if (!gin) return sm[e * T + t];
         return (t < tcount) ? ldstream(src + (size_t)e * pin + p0 + t) : mk(0, 0);
+    }
+    CHAN_HD void prefetch(int e, int t) const {
+#ifdef __CUDA_ARCH__
+        if (t < tcount) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + (size_t)e * pin + p0 + t));
+#endif
     }
     CHAN_HD void store(int e, int t, c2 v) const {
         if (!gout) { sm[e * T + t] = v; return; }
@@ -409,6 +445,7 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true; io.gout = (NS == 1);
+    zprefetch<R0, M0>(io, mz, T, tid, nt);
     zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
     if constexpr (NS > 1) {
         __syncthreads();
@@ -437,6 +474,10 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true;
+    if constexpr (NS > 3) zprefetch<R3, 1>(io, mz, T, tid, nt);
+    else if constexpr (NS > 2) zprefetch<R2, M2>(io, mz, T, tid, nt);
+    else if constexpr (NS > 1) zprefetch<R1, M1>(io, mz, T, tid, nt);
+    else zprefetch<R0, M0>(io, mz, T, tid, nt);
     if constexpr (NS > 3) {
         zpass<R3, false, true, 1>(io, io, P.fz.st[3], mz, T, tid, nt);
         __syncthreads();
