@@ -450,6 +450,9 @@ def main():
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
                 "avg_launch_ms": dms / dcnt, "share_of_step": dms / ms_total}
     if dom == "xfft_prod":
+        roofline["limiter"] = ("latency at 16 warps per SM (registers and shared memory both full with two 256-thread CTAs); "
+                               "ncu: fp64 pipe 49%, issue slots 51%, L1/shared pipe 57%, DRAM 22% -- no unit saturated; the HBM "
+                               "fraction is what north_star asks for, fp64 and smem are the roofs this kernel is nearer to")
         # the x pass is bound by the shared-memory pipe and the fp64 pipe, not by HBM: two more
         # roofs.  "alu": 5 N log2 N flops against the fp64 FMA rate measured by the library's register-only micro-kernel
         # (chan_debug_fma_peak) in this run; "smem": shared-memory wavefronts of one launch (ncu table) x 128 B against

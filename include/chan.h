@@ -177,6 +177,15 @@ int chan_post_sgs(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* d
 #define CHAN_STATS_RESET      4
 int chan_stats(chan_t* h, int flags, double* host_out, long long* nsamples);
 
+/* One-dimensional co-spectra of the current state at every y (NEXT-4 "more statistics"; Fig. 3.1, L163 /
+ * L173 Fig. 3.3 compare such spectra of the database with the reference runs): for the seven second-order quantities
+ * uu,uv,uw,vv,vw,ww, om_i om_i (the order of chan_stats) dev_ex[7][ny][nx/2] = w_p sum over the k_z slots of
+ * Re(a^ conj b^) and dev_ez[7][ny][nz] = sum over p of w_p Re(a^ conj b^) (w_0 = 1, w_p = 2; z slots in FFT order, the
+ * Nyquist slot is zero).  Summed over their wavenumber both equal the plane statistics.  DEVICE outputs, overwritten
+ * (accumulation over snapshots is the caller's); either pointer may be NULL.  Asynchronous on the bound stream.
+ * The friction velocity of L165 (Fig. 3.4) follows from chan_get_scalars(): u_tau^2 = out[2] (bottom wall), out[3] (top). */
+int chan_spectra(chan_t* h, double* dev_ex, size_t ex_bytes, double* dev_ez, size_t ez_bytes);
+
 /* Scalars: out[0] = -dP/dx recovered by the last substep (constant mass flux) or prescribed,
  * out[1] = mass flux Q0, out[2] = nu dU/dy at y=-1, out[3] = -nu dU/dy at y=+1.  Synchronises. */
 int chan_get_scalars(chan_t* h, double* host_out4);

@@ -316,6 +316,21 @@ class ChannelOracle:
         prof[9] = mean(ox, ox) + mean(oy, oy) + mean(oz, oz)
         return prof
 
+    def spectra(self):
+        """One-dimensional co-spectra of the seven second-order quantities uu,uv,uw,vv,vw,ww, om_i om_i at every y
+        (Fig. 3.1, L163/L173 Fig. 3.3 show such spectra of the database): E_x[n][y][p] = w_p sum over k_z
+        slots of Re(a conj b), E_z[n][y][slot] = sum over p of w_p Re(a conj b), w_0 = 1, w_p = 2.  Summed over their
+        wavenumber both give the plane statistics <a b>(y)."""
+        u, v, w, ox, oy, oz = self.velocities_vorticities()
+        wp = np.full(self.nx // 2, 2.0)
+        wp[0] = 1.0
+        pairs = ((u, u), (u, v), (u, w), (v, v), (v, w), (w, w))
+        dens = [(a * np.conj(b)).real for a, b in pairs]
+        dens.append((ox * np.conj(ox)).real + (oy * np.conj(oy)).real + (oz * np.conj(oz)).real)
+        ex = np.stack([np.transpose(wp[:, None] * d.sum(axis=0), (1, 0)) for d in dens])            # [7][ny][nx/2]
+        ez = np.stack([np.transpose(np.einsum("p,qpy->qy", wp, d), (1, 0)) for d in dens])           # [7][ny][nz]
+        return ex, ez
+
     def stats_accumulate(self):
         self.stat_sum += self.stats_profiles()
         self.stat_n += 1

@@ -26,7 +26,7 @@ EXPORTS = [
     "chan_debug_get_band_tables", "chan_debug_launch_count", "chan_debug_transpose",
     "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe", "chan_debug_fma_peak", "chan_set_filter_precision", "chan_run",
     "chan_post_scratch_bytes", "chan_post_pressure", "chan_post_strain_norm", "chan_post_sgs",
-    "chan_mesh_helmholtz_error", "chan_mesh_optimize",
+    "chan_mesh_helmholtz_error", "chan_mesh_optimize", "chan_spectra",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
                   "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged", "post"]
@@ -109,6 +109,7 @@ def load():
         "chan_run": (i, [vp, C.POINTER(Run), C.POINTER(C.c_longlong)]),
         "chan_mesh_helmholtz_error": (i, [i, vp, d, i, vp]),
         "chan_mesh_optimize": (i, [i, vp, i, d, d, i, vp, vp]),
+        "chan_spectra": (i, [vp, vp, sz, vp, sz]),
         "chan_post_scratch_bytes": (sz, [vp, i, i]),
         "chan_post_pressure": (i, [vp, i, i, vp, vp, vp, sz]),
         "chan_post_strain_norm": (i, [vp, i, i, vp, vp, vp, sz]),
@@ -296,6 +297,13 @@ class Channel:
         n = C.c_longlong(0)
         _chk(self.lib.chan_stats(self.h, flags, out.ctypes.data, C.byref(n)), "chan_stats")
         return out, int(n.value)
+
+    def spectra(self):
+        """chan_spectra: (ex [7][ny][nx/2], ez [7][ny][nz]) float64 device tensors."""
+        ex = torch.empty((7, self.ny, self.nx // 2), dtype=torch.float64, device=self.device)
+        ez = torch.empty((7, self.ny, self.nz), dtype=torch.float64, device=self.device)
+        _chk(self.lib.chan_spectra(self.h, ex.data_ptr(), ex.numel() * 8, ez.data_ptr(), ez.numel() * 8), "chan_spectra")
+        return ex, ez
 
     def scalars(self):
         out = np.zeros(4)

@@ -730,6 +730,18 @@ int chan_stats(chan_t* h, int flags, double* host_out, long long* nsamples) {
     return CHAN_OK;
 }
 
+int chan_spectra(chan_t* h, double* dev_ex, size_t ex_bytes, double* dev_ez, size_t ez_bytes) {
+    if (!h || (!dev_ex && !dev_ez)) return CHAN_EINVAL;
+    if (!h->bound || !h->have_state) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if ((dev_ex && ex_bytes < (size_t)7 * P.ny * P.nxh * 8) || (dev_ez && ez_bytes < (size_t)7 * P.ny * P.nz * 8)) return CHAN_ENOSPACE;
+    PlaneParams Q = pparams(h);
+    FieldPtrs in; in.f[0] = h->u; in.f[1] = h->v; in.f[2] = h->w; in.f[3] = h->ox; in.f[4] = h->omy; in.f[5] = h->oz;
+    if (dev_ex) { PB(CHAN_KC_STATS); k_spectra_x<<<dim3((P.nxh + 127) / 128, P.ny), 128, 0, h->stream>>>(Q, in, dev_ex); LAUNCHED(); }
+    if (dev_ez) { PB(CHAN_KC_STATS); k_spectra_z<<<dim3((P.nz + 7) / 8, P.ny), 256, 0, h->stream>>>(Q, in, dev_ez); LAUNCHED(); }
+    return CHAN_OK;
+}
+
 int chan_get_scalars(chan_t* h, double* out4) {
     if (!h || !out4) return CHAN_EINVAL;
     if (!h->bound) return CHAN_ESTATE;

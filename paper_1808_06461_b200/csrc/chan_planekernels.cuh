@@ -70,6 +70,48 @@ __global__ void __launch_bounds__(256) k_stats(PlaneParams P, FieldPtrs in /* u,
 }
 
 // =====================================================================================================
+// One-dimensional co-spectra of uu,uv,uw,vv,vw,ww, om_i om_i at every y (NEXT-4 "more statistics"; PAPER.md L118,
+// L163): ex[7][ny][nxh] = w_p sum over z slots of Re(a conj b), ez[7][ny][nz] = sum over p of w_p Re(a conj b).
+// k_spectra_x: one thread per (y, p), marching over the z slots (consecutive lanes = consecutive p: coalesced);
+// k_spectra_z: one warp per (y, z slot) row, lanes over p, shuffle reduction.  Outputs are overwritten.
+// =====================================================================================================
+__device__ __forceinline__ void cospectra7(const FieldPtrs& in, size_t o, double wgt, double (&s)[7]) {
+    const c2 u = ldc(in.f[0] + o), v = ldc(in.f[1] + o), w = ldc(in.f[2] + o);
+    const c2 ox = ldc(in.f[3] + o), oy = ldc(in.f[4] + o), oz = ldc(in.f[5] + o);
+    s[0] += wgt * (u.x * u.x + u.y * u.y);
+    s[1] += wgt * (u.x * v.x + u.y * v.y);
+    s[2] += wgt * (u.x * w.x + u.y * w.y);
+    s[3] += wgt * (v.x * v.x + v.y * v.y);
+    s[4] += wgt * (v.x * w.x + v.y * w.y);
+    s[5] += wgt * (w.x * w.x + w.y * w.y);
+    s[6] += wgt * (ox.x * ox.x + ox.y * ox.y + oy.x * oy.x + oy.y * oy.y + oz.x * oz.x + oz.y * oz.y);
+}
+__global__ void __launch_bounds__(128) k_spectra_x(PlaneParams P, FieldPtrs in, double* __restrict__ ex) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (p >= P.nxh) return;
+    double s[7] = {0, 0, 0, 0, 0, 0, 0};
+    const size_t off = (size_t)j * P.nm + p;
+    for (int z = 0; z < P.nz; ++z) cospectra7(in, off + (size_t)z * P.nxh, 1.0, s);
+    const double wgt = (p == 0) ? 1.0 : 2.0;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) ex[((size_t)k * P.ny + j) * P.nxh + p] = wgt * s[k];
+}
+__global__ void __launch_bounds__(256) k_spectra_z(PlaneParams P, FieldPtrs in, double* __restrict__ ez) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int z = blockIdx.x * (blockDim.x >> 5) + warp, j = blockIdx.y;
+    if (z >= P.nz) return;
+    double s[7] = {0, 0, 0, 0, 0, 0, 0};
+    const size_t off = (size_t)j * P.nm + (size_t)z * P.nxh;
+    for (int p = lane; p < P.nxh; p += 32) cospectra7(in, off + p, (p == 0) ? 1.0 : 2.0, s);
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        double v = s[k];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) ez[((size_t)k * P.ny + j) * P.nz + z] = v;
+    }
+}
+
+// =====================================================================================================
 // a2 / a8: plain transposes between LINE layout [nm][ny] and PLANE layout [ny][nm] (16-byte elements),
 // 32x32 tiles through shared memory.  dir 0: line -> plane, 1: plane -> line.
 // =====================================================================================================

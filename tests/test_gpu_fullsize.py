@@ -231,6 +231,16 @@ def random_field(shape, nz, seed, dev, scale=1.0):
     return f
 
 
+def _skip_if_whole_config5_fits():
+    """The "cfg5-planes" / "cfg5-lines" cases exercise the plane size and the line length of config 5 on a fraction of its
+    memory; where the device holds the whole config (test_config5_whole_on_sampled_lines_and_planes) they repeat it."""
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    if torch.cuda.mem_get_info(0)[0] >= 170e9 and "cfg5" in (os.environ.get("CHAN_TEST_FULLSIZE") or "cfg5").split(","):
+        pytest.skip("covered by test_config5_whole_on_sampled_lines_and_planes on this device")
+
+
 def fullsize_names():
     """cfg3 and cfg4 by default (about 90 s together); CHAN_TEST_FULLSIZE=cfg3[,cfg4][,cfg5] restricts the list.
     Config 5 has a memory-lean test of its own below (its 148 GB workspace leaves room for one full-size field at a
@@ -245,6 +255,7 @@ def test_fullsize_planes_filter_stats(B, name):
     fields.  "cfg5-planes": the 1536 x 1152 wall-parallel grid of config 5 (its transform plans and tiles) on 72 planes
     with the plane chunks cut down to 11 planes as in the full config 5, so that the seams exist."""
     if name == "cfg5-planes":
+        _skip_if_whole_config5_fits()
         c = inputs.config("cfg5", ny=72)
         tuning = None            # 3 GB chunks = 11 planes of this plane size, as in the full config
     else:
@@ -277,6 +288,7 @@ def test_fullsize_lines_derive_and_ysolve(B, name):
     "cfg5-lines": the 1025-point mesh, Re and dt of config 5 on a 128 x 64 sub-box with the same dx, dz (the same
     range of wavenumbers and Helmholtz parameters, the full line length, every line sampled)."""
     if name == "cfg5-lines":
+        _skip_if_whole_config5_fits()
         c5 = inputs.CONFIGS["cfg5"]
         c = inputs.config("cfg5", nx=128, nz=64, lx=c5["lx"] * 128 / c5["nx"], lz=c5["lz"] * 64 / c5["nz"])
         ps, ss = np.arange(64), np.arange(64)
@@ -350,7 +362,8 @@ def test_config5_whole_on_sampled_lines_and_planes(B):
     torch.cuda.empty_cache()
     free = torch.cuda.mem_get_info(dev)[0]
     if free < 166e9:
-        pytest.skip(f"config 5 needs its 148 GB workspace plus one 14.5 GB field and the filter output on the device ({free / 1e9:.1f} GB free)")
+        pytest.skip(f"config 5 needs its 148 GB workspace plus one 14.5 GB field and the filter output on the device ({free / 1e9:.1f} GB free, "
+                    f"{torch.cuda.memory_allocated(dev) / 1e9:.1f} GB allocated / {torch.cuda.memory_reserved(dev) / 1e9:.1f} GB reserved by this process)")
     hv, hp_, ho = (torch.empty(shape, dtype=torch.complex128) for _ in range(3))
     inputs.fluctuations(c, device=dev, zchunk=16, out=(hv, hp_, ho))
     hU, hW = torch.from_numpy(c["U"]).clone(), torch.from_numpy(c["W"]).clone()

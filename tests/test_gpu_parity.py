@@ -703,3 +703,28 @@ def test_cluster_z_passes_equal_single_cta_z_passes(B, name, tz):
         ch.close()
     for a, b in zip(*res):
         assert rel(a, b.cpu().numpy()) < 1e-13
+
+
+@pytest.mark.parametrize("name", ["cfg1", "mid"])
+def test_spectra(B, name):
+    """chan_spectra (NEXT-4) against oracle.spectra, and its consistency with chan_stats."""
+    c, ch, o = make(B, name)
+    v, phi, omy = seeded_state(c, 20.0 if name == "cfg1" else 1.0)
+    ch.set_state(v, phi, omy, c["U"], c["W"])
+    o.set_state(v, phi, omy, c["U"], c["W"])
+    ch.step()
+    o.step()
+    ex, ez = (t.cpu().numpy() for t in ch.spectra())
+    rx, rz = o.spectra()
+    for n in range(7):
+        assert np.abs(ex[n] - rx[n]).max() < 1e-10 * np.abs(rx[n]).max(), n
+        assert np.abs(ez[n] - rz[n]).max() < 1e-10 * np.abs(rz[n]).max(), n
+    ch.stats(B.STATS_RESET | B.STATS_ACCUMULATE)
+    prof, _ = ch.stats(B.STATS_READ)
+    for n in range(7):
+        sc = max(1.0, np.abs(prof[3 + n]).max())
+        assert np.abs(ex[n].sum(axis=1) - prof[3 + n]).max() < 1e-12 * sc and np.abs(ez[n].sum(axis=1) - prof[3 + n]).max() < 1e-12 * sc
+    small = torch.empty(8, dtype=torch.float64, device="cuda")
+    assert ch.lib.chan_spectra(ch.h, small.data_ptr(), 64, None, 0) == B.ENOSPACE
+    assert ch.lib.chan_spectra(ch.h, None, 0, None, 0) == B.EINVAL
+    ch.close()

@@ -131,3 +131,35 @@ def test_run_emits_snapshots_at_the_cadence():
     assert np.array_equal(o.stats_read()[0], ref.stats_read()[0]) and o.stats_read()[1] == 5
     assert np.array_equal(o.v, ref.v)
     assert o.run(2, 0, 0, *c["cut"]) == []
+
+
+def test_spectra_sum_to_the_statistics_and_match_physical_space_transforms():
+    """oracle.spectra (NEXT-4 "more statistics"): summed over their wavenumber the co-spectra are
+    the plane statistics; and E_x of uu, vw equals the z-average of the one-dimensional x-transform of the PHYSICAL
+    fields on the dealiased grid (an evaluation that never touches the spectral weights w_p), likewise E_z."""
+    c, o = _setup()
+    ex, ez = o.spectra()
+    prof = o.stats_profiles()
+    assert ex.shape == (7, o.ny, o.nx // 2) and ez.shape == (7, o.ny, o.nz)
+    for n in range(7):
+        sc = max(1.0, np.abs(prof[3 + n]).max())
+        assert np.abs(ex[n].sum(axis=1) - prof[3 + n]).max() < 1e-12 * sc
+        assert np.abs(ez[n].sum(axis=1) - prof[3 + n]).max() < 1e-12 * sc
+    assert not ez[:, :, o.nz // 2].any()                                  # the z-Nyquist slot carries nothing
+    u, v, w = (o.to_physical(f) for f in o.velocities_vorticities()[:3])     # [ny][mz][mx]
+    mx, mz = o.mx, o.mz
+    for n, (a, b) in ((0, (u, u)), (4, (v, w))):
+        fa, fb = np.fft.fft(a, axis=2) / mx, np.fft.fft(b, axis=2) / mx     # full complex x-transform, all mx modes
+        co = (fa * np.conj(fb)).real.mean(axis=1)                           # z-average -> [ny][mx]
+        half = co[:, : o.nx // 2].copy()
+        half[:, 1:] += co[:, :-(o.nx // 2):-1][:, : o.nx // 2 - 1]          # fold -p onto p
+        assert np.abs(half - ex[n]).max() < 1e-12 * np.abs(ex[n]).max()
+        ga, gb = np.fft.fft(a, axis=1) / mz, np.fft.fft(b, axis=1) / mz
+        cz = (ga * np.conj(gb)).real.mean(axis=2)                           # x-average -> [ny][mz]
+        slots = [q % mz for q in o.q]
+        zz = cz[:, slots]
+        zz[:, o.nz // 2] = 0.0
+        # a real field's (-p, k_z) mode is the conjugate of (p, -k_z): the physical z-spectrum at k_z holds half of the
+        # spectral weight-2 sums at k_z and half of those at -k_z, so compare the +-k_z pairs
+        mirror = [list(o.q).index(-q) if s_ != o.nz // 2 else s_ for s_, q in enumerate(o.q)]
+        assert np.abs((zz + zz[:, mirror]) - (ez[n] + ez[n][:, mirror])).max() < 1e-12 * np.abs(ez[n]).max()
