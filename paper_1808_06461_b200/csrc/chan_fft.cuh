@@ -302,8 +302,9 @@ struct ZInvIO {
     const double2* src;             // plane of the field: [nz][nxh]
     double2* dst;                   // plane of zpad: [mz][nxh]
     int nxh, nzh, nz, mz, p0, tcount;
+    bool zband = false;             // shared-memory reads of the zero band of the 3/2 padding (never filled) return zero
     CHAN_HD c2 load(int e, int t) const {
-        if (!gin) return sm[e * T + t];
+        if (!gin) return (zband && e >= nzh && e <= mz - nzh) ? mk(0, 0) : sm[e * T + t];
         int s = -1;
         if (e < nzh) s = e; else if (e > mz - nzh) s = e - (mz - nz);
         return (s >= 0 && t < tcount) ? ldstream(src + (size_t)s * nxh + p0 + t) : mk(0, 0);
@@ -433,6 +434,20 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_g(CHAN_ZARGS_FWD) {
     }
 }
 
+// Asynchronous tile fill (cp.async, 16 bytes per copy, L1 bypassed): the stage that used to read global memory into
+// registers, one butterfly at a time, exposed one memory latency per butterfly round and was half of the z passes'
+// time (ncu source view: 44-58% of its samples on the first use of a loaded value).  Every thread now queues the copies of
+// the WHOLE tile into its final shared-memory rows up front -- no registers held, 70-110 KB in flight per CTA -- and the
+// first stage runs out of shared memory like the others.
+#ifndef CHAN_ZASYNC
+#define CHAN_ZASYNC 1
+#endif
+__device__ __forceinline__ void cp_async16(void* smem, const void* g) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory"); }
+
 // Bodies with explicit block coordinates (bx = column tile, jc = plane of the chunk, fi = field), shared by the
 // stand-alone kernels below and by the merged plane kernel k_planes_s.
 template <int R0, int R1, int R2, int R3>
@@ -444,9 +459,28 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
                              zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
-    io.gin = true; io.gout = (NS == 1);
-    zprefetch<R0, M0>(io, mz, T, tid, nt);
-    zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
+    if constexpr (CHAN_ZASYNC && NS > 1) {
+        // retained rows s != nzh of the field -> rows e(s) of the tile; columns beyond a ragged tile are zero-filled
+        int lgT = 0;
+        while ((1 << lgT) < T) ++lgT;
+        c2* sm = io.sm;
+        for (int w = tid; w < (P.nz << lgT); w += nt) {
+            const int sl = w >> lgT, t = w & (T - 1);
+            if (sl == P.nzh) continue;
+            const int e = sl < P.nzh ? sl : sl + (mz - P.nz);
+            if (t < io.tcount) cp_async16(sm + e * T + t, io.src + (size_t)sl * P.nxh + p0 + t);
+            else sm[e * T + t] = mk(0, 0);
+        }
+        cp_async_wait_all();
+        __syncthreads();
+        io.gin = false; io.gout = false; io.zband = true;
+        zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
+        io.zband = false;
+    } else {
+        io.gin = true; io.gout = (NS == 1);
+        zprefetch<R0, M0>(io, mz, T, tid, nt);
+        zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
+    }
     if constexpr (NS > 1) {
         __syncthreads();
         io.gin = false; io.gout = (NS == 2);
@@ -474,7 +508,19 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true;
-    if constexpr (NS > 3) zprefetch<R3, 1>(io, mz, T, tid, nt);
+    if constexpr (CHAN_ZASYNC && NS > 1) {
+        int lgT = 0;
+        while ((1 << lgT) < T) ++lgT;
+        c2* sm = io.sm;
+        for (int w = tid; w < (mz << lgT); w += nt) {
+            const int e = w >> lgT, t = w & (T - 1);
+            if (t < io.tcount) cp_async16(sm + e * T + t, io.src + (size_t)e * pin + p0 + t);
+            else sm[e * T + t] = mk(0, 0);
+        }
+        cp_async_wait_all();
+        __syncthreads();
+        io.gin = false;
+    } else if constexpr (NS > 3) zprefetch<R3, 1>(io, mz, T, tid, nt);
     else if constexpr (NS > 2) zprefetch<R2, M2>(io, mz, T, tid, nt);
     else if constexpr (NS > 1) zprefetch<R1, M1>(io, mz, T, tid, nt);
     else zprefetch<R0, M0>(io, mz, T, tid, nt);
