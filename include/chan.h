@@ -204,7 +204,7 @@ typedef struct {
     int maxradix_z;       /* 2..12: largest radix of a z stage                                                    */
     int maxradix_x;       /* 2..18: largest radix of an x stage in front of the fused one                          */
     int tz;               /* k_x columns per z tile: 1, 2, 4, 8 or 16                                              */
-    int zthreads;         /* threads per CTA of the z passes, 32..256                                              */
+    int zthreads;         /* threads per CTA of the z passes, a multiple of 32 in 32..256                          */
     int xthreads;         /* threads per CTA of the x pass, 32..256                                                */
     int chunk_mb;         /* size of the z-padded plane-chunk buffers in MiB (default 3072)                        */
     int planes_per_chunk; /* get only: y-planes per launch of the plane kernels that follows from chunk_mb         */

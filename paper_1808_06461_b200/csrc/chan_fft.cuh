@@ -446,6 +446,29 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* g) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(g) : "memory");
 }
+// CHAN_ZASYNC == 2 (measured, not the default): the same fill with one bulk copy per ROW PIECE (cp.async.bulk, T x 16
+// contiguous bytes, completion counted in bytes on an mbarrier).  UBLKCP is a warp-uniform instruction: the compiler
+// serialises the 32 lanes of a warp (ELECT / R2UR loop), and 64-byte pieces are too small to pay for that: K2 53 -> 62 ms,
+// K4 30 -> 44 ms on config 5.  A strided tile wants a tensor map (one instruction per 256-row box), not 1-D bulk copies.
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n\tfence.mbarrier_init.release.cluster;" ::"r"(a), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem, const void* g, unsigned bytes, unsigned long long* bar) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem), a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(d), "l"(g), "r"(bytes), "r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory"); }
 
 // Bodies with explicit block coordinates (bx = column tile, jc = plane of the chunk, fi = field), shared by the
@@ -461,17 +484,38 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
     const int tid = threadIdx.x, nt = blockDim.x;
     if constexpr (CHAN_ZASYNC && NS > 1) {
         // retained rows s != nzh of the field -> rows e(s) of the tile; columns beyond a ragged tile are zero-filled
-        int lgT = 0;
-        while ((1 << lgT) < T) ++lgT;
         c2* sm = io.sm;
-        for (int w = tid; w < (P.nz << lgT); w += nt) {
-            const int sl = w >> lgT, t = w & (T - 1);
-            if (sl == P.nzh) continue;
-            const int e = sl < P.nzh ? sl : sl + (mz - P.nz);
-            if (t < io.tcount) cp_async16(sm + e * T + t, io.src + (size_t)sl * P.nxh + p0 + t);
-            else sm[e * T + t] = mk(0, 0);
+        if constexpr (CHAN_ZASYNC == 2) {
+            __shared__ unsigned long long mbar;
+            const unsigned rowbytes = (unsigned)io.tcount * 16u;
+            if (tid == 0) mbar_init(&mbar, 1);
+            __syncthreads();
+            if (tid == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(P.nz - 1) * rowbytes);
+            for (int sl = tid; sl < P.nz; sl += nt) {
+                if (sl == P.nzh) continue;
+                const int e = sl < P.nzh ? sl : sl + (mz - P.nz);
+                bulk_g2s(sm + e * T, io.src + (size_t)sl * P.nxh + p0, rowbytes, &mbar);
+                for (int t = io.tcount; t < T; ++t) sm[e * T + t] = mk(0, 0);
+            }
+            mbar_wait(&mbar, 0);
+        } else {
+            // thread = (column t, row r0 + i rs): pointer increments only inside the loops; low band, then high band
+            int lgT = 0;
+            while ((1 << lgT) < T) ++lgT;
+            const int t = tid & (T - 1), r0 = tid >> lgT, rs = nt >> lgT;        // nt is a multiple of 32 >= T
+            const bool live = t < io.tcount;
+            const double2* g = io.src + (size_t)r0 * P.nxh + p0 + t;
+            c2* d = sm + r0 * T + t;
+            const size_t gs = (size_t)rs * P.nxh;
+            const int ds = rs * T;
+#pragma unroll 4
+            for (int sl = r0; sl < P.nzh; sl += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
+            g = io.src + (size_t)(P.nzh + 1 + r0) * P.nxh + p0 + t;
+            d = sm + (P.nzh + 1 + r0 + (mz - P.nz)) * T + t;
+#pragma unroll 4
+            for (int sl = P.nzh + 1 + r0; sl < P.nz; sl += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
+            cp_async_wait_all();
         }
-        cp_async_wait_all();
         __syncthreads();
         io.gin = false; io.gout = false; io.zband = true;
         zpass<R0, true, false, M0>(io, io, P.fz.st[0], mz, T, tid, nt);
@@ -509,15 +553,31 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
     const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true;
     if constexpr (CHAN_ZASYNC && NS > 1) {
-        int lgT = 0;
-        while ((1 << lgT) < T) ++lgT;
         c2* sm = io.sm;
-        for (int w = tid; w < (mz << lgT); w += nt) {
-            const int e = w >> lgT, t = w & (T - 1);
-            if (t < io.tcount) cp_async16(sm + e * T + t, io.src + (size_t)e * pin + p0 + t);
-            else sm[e * T + t] = mk(0, 0);
+        if constexpr (CHAN_ZASYNC == 2) {
+            __shared__ unsigned long long mbar;
+            const unsigned rowbytes = (unsigned)io.tcount * 16u;
+            if (tid == 0) mbar_init(&mbar, 1);
+            __syncthreads();
+            if (tid == 0) mbar_arrive_expect_tx(&mbar, (unsigned)mz * rowbytes);
+            for (int e = tid; e < mz; e += nt) {
+                bulk_g2s(sm + e * T, io.src + (size_t)e * pin + p0, rowbytes, &mbar);
+                for (int t = io.tcount; t < T; ++t) sm[e * T + t] = mk(0, 0);
+            }
+            mbar_wait(&mbar, 0);
+        } else {
+            int lgT = 0;
+            while ((1 << lgT) < T) ++lgT;
+            const int t = tid & (T - 1), r0 = tid >> lgT, rs = nt >> lgT;
+            const bool live = t < io.tcount;
+            const double2* g = io.src + (size_t)r0 * pin + p0 + t;
+            c2* d = sm + r0 * T + t;
+            const size_t gs = (size_t)rs * pin;
+            const int ds = rs * T;
+#pragma unroll 4
+            for (int e = r0; e < mz; e += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
+            cp_async_wait_all();
         }
-        cp_async_wait_all();
         __syncthreads();
         io.gin = false;
     } else if constexpr (NS > 3) zprefetch<R3, 1>(io, mz, T, tid, nt);
