@@ -471,7 +471,7 @@ int chan_debug_set_tuning(chan_t* h, const chan_tuning_t* t) {
     auto pow2 = [](int v) { return v == 1 || v == 2 || v == 4 || v == 8 || v == 16; };
     if ((t->xfuse && t->xfuse != 4 && t->xfuse != 8) || (t->maxradix_z && (t->maxradix_z < 2 || t->maxradix_z > 12)) ||
         (t->maxradix_x && (t->maxradix_x < 2 || t->maxradix_x > 18)) || (t->tz && !pow2(t->tz)) ||
-        (t->zthreads && (t->zthreads < 32 || t->zthreads > 256 || t->zthreads % 32)) || (t->xthreads && (t->xthreads < 32 || t->xthreads > 256)) ||
+        (t->zthreads && (t->zthreads < 32 || t->zthreads > 256 || t->zthreads % 32)) || (t->xthreads && (t->xthreads < 32 || t->xthreads > CHAN_XNT)) ||
         t->chunk_mb < 0 || t->plane_overlap < 0 || t->plane_overlap > 2 || t->z_cluster < 0 || t->z_cluster > 2)
         return CHAN_EINVAL;
     const chan_tuning_t old = h->tune;

@@ -821,27 +821,32 @@ CHAN_HD void xfused(const XIO& io, int n, int tid, int nt) {
 
 CHAN_HD void xpack(const XIO& io, int mx, int nxh, const double2* zrow, size_t fstride, int tid, int nt, bool fill_zero) {
     // C[k] = A[k] + i B[k], C[mx-k] = conj(A[k]) + i conj(B[k]); Im of the k = 0 entries dropped (R14).
-    // The global loads of XB work items are issued before the first shared-memory store: one exposed memory latency
-    // per XB items instead of one per item (a 768-column row is 9 items per thread at 256 threads).
-    constexpr int XB = 5;
-    const int total = 3 * nxh;
-    for (int w0 = tid; w0 < total; w0 += nt * XB) {
-        c2 A[XB], B[XB];
+    // A thread owns columns k = tid + i nt of all three pairs: no index division, and the global loads of XK columns
+    // (6 XK loads of 16 bytes) are issued before the first shared-memory store -- the pack was 29% of the x pass
+    // (ncu source view), most of it waiting on two or three rounds of loads and on integer divisions.
+    constexpr int XK = 3;
+    for (int k0 = tid; k0 < nxh; k0 += nt * XK) {
+        c2 A[XK][3], B[XK][3];
 #pragma unroll
-        for (int i = 0; i < XB; ++i) {
-            const int w = w0 + i * nt;
-            if (w < total) {
-                const int pr = w / nxh, k = w - pr * nxh;
-                A[i] = ldstream(zrow + (size_t)(2 * pr) * fstride + k); B[i] = ldstream(zrow + (size_t)(2 * pr + 1) * fstride + k);
+        for (int i = 0; i < XK; ++i) {
+            const int k = k0 + i * nt;
+            if (k < nxh) {
+#pragma unroll
+                for (int pr = 0; pr < 3; ++pr) {
+                    A[i][pr] = ldstream(zrow + (size_t)(2 * pr) * fstride + k); B[i][pr] = ldstream(zrow + (size_t)(2 * pr + 1) * fstride + k);
+                }
             }
         }
 #pragma unroll
-        for (int i = 0; i < XB; ++i) {
-            const int w = w0 + i * nt;
-            if (w < total) {
-                const int pr = w / nxh, k = w - pr * nxh;
-                if (k == 0) io.store(0, pr, mk(A[i].x, B[i].x));
-                else { io.store(k, pr, mk(A[i].x - B[i].y, A[i].y + B[i].x)); io.store(mx - k, pr, mk(A[i].x + B[i].y, -A[i].y + B[i].x)); }
+        for (int i = 0; i < XK; ++i) {
+            const int k = k0 + i * nt;
+            if (k < nxh) {
+#pragma unroll
+                for (int pr = 0; pr < 3; ++pr) {
+                    const c2 a = A[i][pr], b = B[i][pr];
+                    if (k == 0) io.store(0, pr, mk(a.x, b.x));
+                    else { io.store(k, pr, mk(a.x - b.y, a.y + b.x)); io.store(mx - k, pr, mk(a.x + b.y, -a.y + b.x)); }
+                }
             }
         }
     }
@@ -855,11 +860,13 @@ template <int NPROD>
 CHAN_HD void xunpack(const XIO& io, int mx, double2* xrow, size_t ostride, int pout, int tid, int nt) {
     constexpr int NC = (NPROD + 1) / 2;
     // A[k] = (D[k] + conj D[mx-k])/2, B[k] = (D[k] - conj D[mx-k])/(2i)
-    for (int w = tid; w < NC * pout; w += nt) {
-        const int pr = w / pout, k = w - pr * pout;
-        const c2 d = io.load(k, pr), e = io.load(k == 0 ? 0 : mx - k, pr);
-        ststream(xrow + (size_t)(2 * pr) * ostride + k, mk(0.5 * (d.x + e.x), 0.5 * (d.y - e.y)));
-        if (2 * pr + 1 < NPROD) ststream(xrow + (size_t)(2 * pr + 1) * ostride + k, mk(0.5 * (d.y + e.y), -0.5 * (d.x - e.x)));
+    for (int k = tid; k < pout; k += nt) {
+#pragma unroll
+        for (int pr = 0; pr < NC; ++pr) {
+            const c2 d = io.load(k, pr), e = io.load(k == 0 ? 0 : mx - k, pr);
+            ststream(xrow + (size_t)(2 * pr) * ostride + k, mk(0.5 * (d.x + e.x), 0.5 * (d.y - e.y)));
+            if (2 * pr + 1 < NPROD) ststream(xrow + (size_t)(2 * pr + 1) * ostride + k, mk(0.5 * (d.y + e.y), -0.5 * (d.x - e.x)));
+        }
     }
 }
 
@@ -931,8 +938,11 @@ __device__ __forceinline__ void xprod_body(const PlaneParams& P, const double2* 
     if constexpr (R0 > 1) { io.zout = true; xpass<R0, false, true, M0>(io, P.fx.st[0], mx, NC, tid, nt); io.zout = false; __syncthreads(); }
     xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
 }
+#ifndef CHAN_XNT
+#define CHAN_XNT 256      // most threads of an x-pass CTA (two CTAs per SM)
+#endif
 template <int NPROD, int F, int R0, int R1, int R2>
-__global__ void __launch_bounds__(NPROD == 7 ? 512 : 256, NPROD == 7 ? 1 : 2) k_xfft_prod_s(CHAN_XARGS) {
+__global__ void __launch_bounds__(NPROD == 7 ? 512 : CHAN_XNT, NPROD == 7 ? 1 : 2) k_xfft_prod_s(CHAN_XARGS) {
     extern __shared__ double2 smem_raw[];
     xprod_body<NPROD, F, R0, R1, R2>(P, zpad, npl, xh, pout, smem_raw, blockIdx.x, blockIdx.y);
 }
