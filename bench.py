@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the channel-flow hot path on B200 (metric: BASELINE.json).
 
-A "step" is one pass of the whole hot path over one synthetic field: one chan_stats accumulate (a14) and
-one chan_step_filter = the filtered database of the entry state (a13) fused into one full RK3 step
+A "step" is one pass of the whole hot path over one synthetic field: chan_run over one step with snapshot and
+statistics cadence 1 = the plane statistics (a14) and the filtered database of the entry state (a13) fused into one full RK3 step
 (3 substeps = rows a1-a12 of DESIGN.md).  ``value`` counts only the 3 substeps' grid points (Mpoint*RK-substeps/s), so the
 filter and statistics time is inside the denominator but earns no credit; ``substep_only`` gives the
 rate of the substeps alone.  Inputs are resident in HBM before the timed region; ``e2e`` repeats the
@@ -379,12 +379,13 @@ def main():
     ch.set_state_host(hv, hp, ho, hU, hW)
     fout = torch.empty((10, c["ny"], 2 * kzc + 1, kxc + 1), dtype=torch.complex128, device=dev)
     stream = ch.stream
+    fring = fout.unsqueeze(0)            # a ring of one slot over the same memory
 
     def one_step():
         # statistics and filtered database of the state the step starts from, then the step: chan_step_filter forms the
         # filter products from the z-padded planes of the first substep (no inverse z sweep of its own)
-        ch.stats(binding.STATS_ACCUMULATE)
-        ch.step_filter(kxc, kzc, fout)
+        # (chan_run with every = 1: the statistics come out of the (0,0) modes of the fp64 database it writes, L124)
+        ch.run(1, 1, 1, kxc, kzc, ring=fring)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -493,8 +494,8 @@ def main():
 
             def e2e_step():
                 ch.set_state_host(hv, hp, ho, hU, hW)
-                ch.stats(binding.STATS_ACCUMULATE | binding.STATS_READ)
-                ch.step_filter(kxc, kzc, fout)
+                ch.run(1, 1, 1, kxc, kzc, ring=fring)
+                ch.stats(binding.STATS_READ)
                 with torch.cuda.stream(stream):
                     hf.copy_(fout)                      # the filtered database back to pinned host memory
                 ch.get_state_host(hv, hp, ho, hU, hW)
@@ -514,7 +515,7 @@ def main():
             e2e = {"value": job_value(npts, 3 * Ke, world, ms_e), "unit": UNIT, "steps": Ke,
                    "ms_per_step": ms_e / Ke, "h2d_bytes_per_step": state_b,
                    "d2h_bytes_per_step": state_b + hf.numel() * 16 + 10 * c["ny"] * 8,
-                   "api": "chan_set_state_host + chan_stats(READ) + chan_step_filter + database D2H + chan_get_state_host, "
+                   "api": "chan_set_state_host + chan_run(1 step, database + statistics) + chan_stats(READ) + database D2H + chan_get_state_host, "
                           + ("pinned" if pinned else "pageable (pinning refused)") + " host buffers"}
             del hf
         except RuntimeError as ex:      # pinned allocation refused by the host
@@ -551,7 +552,7 @@ def main():
         "ms_per_step": ms_total_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl, "grid": [c["nx"], c["ny"], c["nz"]], "padded": [3 * c["nx"] // 2, c["ny"], 3 * c["nz"] // 2],
-                   "step": "chan_stats(ACCUMULATE) + chan_step_filter (= chan_filter_store of the entry state + 1 RK3 step of 3 substeps); value counts the 3 substeps",
+                   "step": "chan_run(nsteps=1, filter_every=1, stats_every=1) = statistics + filtered database of the entry state (chan_filter_store fused into the step) + 1 RK3 step of 3 substeps; value counts the 3 substeps",
                    "filter_cut": [kxc, kzc], "l2": "inputs larger than L2 (one field = %.2f GB)" % (F / 1e9),
                    "workspace_GB": ws_bytes / 1e9, "multi_gpu": "replicas only", "state_finite": finite, "plan": plan_text,
                    "tuning": tune},

@@ -118,7 +118,10 @@ int chan_set_filter_precision(chan_t* h, int bytes_per_real);
  * (emitted so far) % ring_slots of dev_ring if filter_every > 0 and n % filter_every == 0.  A slot is slot_bytes
  * long and must hold one database in the precision in effect (CHAN_ENOSPACE otherwise); the caller drains the ring
  * (e.g. by copies on another stream ordered by events) before it wraps.  *snapshots = databases emitted (may be
- * NULL).  Everything is enqueued on the bound stream; nothing synchronises.  CHAN_ESTATE mid-step. */
+ * NULL).  Everything is enqueued on the bound stream; nothing synchronises.  CHAN_ESTATE mid-step.
+ * When the statistics and an fp64 database fall on the same step, the ten profiles are taken from the (0,0) modes of
+ * that database -- which ARE the plane statistics of the full field (L124: second-order consistent) -- instead of a
+ * pass over the fields of their own: equal to chan_stats(ACCUMULATE) to rounding. */
 typedef struct {
     int nsteps, filter_every, stats_every;
     int kx_cut, kz_cut;

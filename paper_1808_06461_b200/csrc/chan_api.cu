@@ -707,10 +707,18 @@ int chan_run(chan_t* h, const chan_run_t* r, long long* snapshots) {
     long long emitted = 0;
     for (int n = 0; n < r->nsteps; ++n) {
         int rc;
-        if (r->stats_every > 0 && n % r->stats_every == 0 && (rc = chan_stats(h, CHAN_STATS_ACCUMULATE, nullptr, nullptr))) return rc;
-        if (r->filter_every > 0 && n % r->filter_every == 0) {
+        const bool st = r->stats_every > 0 && n % r->stats_every == 0, fl = r->filter_every > 0 && n % r->filter_every == 0;
+        // statistics of a step that also emits an fp64 database come out of that database's (0,0) modes
+        const bool st_db = st && fl && !h->out_f32;
+        if (st && !st_db && (rc = chan_stats(h, CHAN_STATS_ACCUMULATE, nullptr, nullptr))) return rc;
+        if (fl) {
             char* slot = (char*)r->dev_ring + (size_t)(emitted % r->ring_slots) * r->slot_bytes;
             if ((rc = step_filter_impl(h, r->kx_cut, r->kz_cut, slot, r->slot_bytes))) return rc;
+            if (st_db) {
+                const size_t plane = (size_t)(2 * r->kz_cut + 1) * (r->kx_cut + 1);
+                PB(CHAN_KC_STATS); k_stats_from_db<<<(10 * h->P.ny + 255) / 256, 256, 0, h->stream>>>(h->P.ny, plane, (const double2*)slot, h->stats); LAUNCHED();
+                ++h->nsamples;
+            }
             ++emitted;
         } else if ((rc = chan_step(h))) return rc;
     }

@@ -70,6 +70,16 @@ __global__ void __launch_bounds__(256) k_stats(PlaneParams P, FieldPtrs in /* u,
 }
 
 // =====================================================================================================
+// a14 from a database just written (fp64): the (0,0) mode of the ten stored variables IS the plane statistics of
+// the full field (second-order consistency) -- no pass over the fields.  acc[10][ny] += Re db[n][j][0][0].
+// =====================================================================================================
+__global__ void k_stats_from_db(int ny, size_t plane, const double2* __restrict__ db, double* __restrict__ acc) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= 10 * ny) return;
+    acc[e] += db[(size_t)e * plane].x;
+}
+
+// =====================================================================================================
 // One-dimensional co-spectra of uu,uv,uw,vv,vw,ww, om_i om_i at every y (NEXT-4 "more statistics"; PAPER.md L118,
 // L163): ex[7][ny][nxh] = w_p sum over z slots of Re(a conj b), ez[7][ny][nz] = sum over p of w_p Re(a conj b).
 // k_spectra_x: one thread per (y, p), marching over the z slots (consecutive lanes = consecutive p: coalesced);

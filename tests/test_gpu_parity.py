@@ -609,7 +609,11 @@ def test_run_cadence_equals_the_calls_written_out(B, single):
         assert torch.equal(x, y)
     sa, na = a.stats(B.STATS_READ)
     sb, nb = b.stats(B.STATS_READ)
-    assert na == nb == 5 and np.array_equal(sa, sb)
+    assert na == nb == 5
+    if single:
+        assert np.array_equal(sa, sb)                  # binary32 database: the statistics keep their own pass
+    else:                                              # fp64 database: taken from its (0,0) modes on the emitting steps
+        assert np.abs(sa - sb).max() < 1e-13 * np.abs(sb).max()
     snaps = o.run(5, 2, 1, kxc, kzc, single=single)
     so, no = o.stats_read()
     assert no == 5 and np.abs(sa - so).max() < 1e-10 * np.abs(so).max()
