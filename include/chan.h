@@ -35,6 +35,7 @@ extern "C" {
 #define CHAN_ENOSPACE -2  /* workspace or output buffer too small                                   */
 #define CHAN_ESTATE   -3  /* wrong call order (not bound, no state, chan_step() mid-step)           */
 #define CHAN_ECUDA    -4  /* a CUDA runtime call or kernel launch failed                            */
+#define CHAN_ELIMIT   -5  /* problem larger than the fixed static scratch of chan_post_strain_norm_static */
 
 typedef struct chan chan_t; /* opaque */
 
@@ -165,6 +166,20 @@ size_t chan_post_scratch_bytes(const chan_t* h, int kx_cut, int kz_cut);
 int chan_post_pressure(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* dev_p, void* dev_scratch, size_t scratch_bytes);
 /* Filtered S_ij S_ij = d_ij(u_i u_j) + om_i om_i / 2: identity (3.3) of L134 as re-derived in reading R17. */
 int chan_post_strain_norm(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* dev_out, void* dev_scratch, size_t scratch_bytes);
+/* chan_post_strain_norm for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same kernel and the same result, bit for bit, but the one scratch plane set lives in a
+ * file-scope `static __device__` array of CHAN_STATIC_SCRATCH_BYTES (4 MiB) inside the library -- every GPU that loads
+ * libchan.so holds those 4 MiB until the process exits.  The caller passes only the database and the output; the call
+ * allocates nothing (no cudaMalloc / cudaFree / allocating library routine, on the host one device-address lookup per
+ * device on first use) and enqueues one kernel on the bound stream.
+ * Limit: ny (2 kz_cut + 1)(kx_cut + 1) * 16 bytes <= CHAN_STATIC_SCRATCH_BYTES, i.e. 262144 stored (y, mode) points;
+ * beyond it CHAN_ELIMIT and nothing is launched -- use chan_post_strain_norm with caller scratch then.
+ * The array is SHARED by every call, handle and stream of the process on that GPU and keeps the last call's contents:
+ * nothing in it needs to start at zero (each mode writes its column before reading it), but two calls that overlap on
+ * the GPU (different streams, or different handles bound to different streams) race on it.  Calls on one stream are safe. */
+#define CHAN_STATIC_SCRATCH_BYTES (4u << 20)
+size_t chan_post_strain_norm_static_limit(void);     /* = CHAN_STATIC_SCRATCH_BYTES */
+int chan_post_strain_norm_static(chan_t* h, int kx_cut, int kz_cut, const void* dev_db, void* dev_out);
 /* Sub-grid stresses (3.4), L149: dev_tau[6][ny][2 kz_cut+1][kx_cut+1] = stored u_i u_j minus the product of the STORED
  * velocities, formed by the library's dealiased product path on this handle's grid and pruned to the cutoff (R20),
  * order uu,uv,uw,vv,vw,ww.  Overwrites the handle's derived fields u, w, om_x, om_z and rebuilds them (step a1) if the

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libchan.so")
 _lib = None
 
-OK, EINVAL, ENOSPACE, ESTATE, ECUDA = 0, -1, -2, -3, -4
+OK, EINVAL, ENOSPACE, ESTATE, ECUDA, ELIMIT = 0, -1, -2, -3, -4, -5
 STATS_ACCUMULATE, STATS_READ, STATS_RESET = 1, 2, 4
 F_V, F_PHI, F_OMY, F_U, F_W, F_OMX, F_OMZ, F_H1, F_H2, F_H3, F_HV_PREV, F_HG_PREV = range(12)
 STAGE_DERIVE, STAGE_NONLINEAR, STAGE_YSOLVE = range(3)
@@ -27,6 +27,7 @@ EXPORTS = [
     "chan_debug_profile", "chan_debug_profile_read", "chan_debug_set_tuning", "chan_debug_get_tuning", "chan_debug_describe", "chan_debug_fma_peak", "chan_set_filter_precision", "chan_run",
     "chan_post_scratch_bytes", "chan_post_pressure", "chan_post_strain_norm", "chan_post_sgs",
     "chan_mesh_helmholtz_error", "chan_mesh_optimize", "chan_spectra",
+    "chan_post_strain_norm_static", "chan_post_strain_norm_static_limit",
 ]
 KERNEL_CLASSES = ["d1_forward", "derive_down", "derive_up", "zfft_inv", "xfft_prod", "zfft_fwd", "mean", "y1", "y2", "y3",
                   "y4", "y5", "transpose", "filter_copy", "xfft_prod_filter", "zfft_fwd_filter", "stats", "planes_merged", "post"]
@@ -114,6 +115,8 @@ def load():
         "chan_post_pressure": (i, [vp, i, i, vp, vp, vp, sz]),
         "chan_post_strain_norm": (i, [vp, i, i, vp, vp, vp, sz]),
         "chan_post_sgs": (i, [vp, i, i, vp, vp, vp, sz]),
+        "chan_post_strain_norm_static": (i, [vp, i, i, vp, vp]),
+        "chan_post_strain_norm_static_limit": (sz, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -288,6 +291,13 @@ class Channel:
 
     def post_strain_norm(self, kx_cut, kz_cut, db):
         return self._post(self.lib.chan_post_strain_norm, "chan_post_strain_norm", kx_cut, kz_cut, db)
+
+    def post_strain_norm_static(self, kx_cut, kz_cut, db, out):
+        """chan_post_strain_norm_static: caller-owned ``out``; the scratch is the library's static device array."""
+        assert db.dtype == torch.complex128 and db.is_contiguous() and out.dtype == torch.complex128 and out.is_contiguous()
+        assert tuple(out.shape) == (self.ny, 2 * kz_cut + 1, kx_cut + 1)
+        _chk(self.lib.chan_post_strain_norm_static(self.h, kx_cut, kz_cut, db.data_ptr(), out.data_ptr()), "chan_post_strain_norm_static")
+        return out
 
     def post_sgs(self, kx_cut, kz_cut, db):
         return self._post(self.lib.chan_post_sgs, "chan_post_sgs", kx_cut, kz_cut, db, lead=(6,))

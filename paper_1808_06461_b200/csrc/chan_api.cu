@@ -5,6 +5,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -785,6 +786,7 @@ const char* chan_strerror(int s) {
         case CHAN_ENOSPACE: return "workspace or output buffer too small";
         case CHAN_ESTATE: return "call out of order";
         case CHAN_ECUDA: return "CUDA error";
+        case CHAN_ELIMIT: return "problem larger than the static scratch limit of this entry point";
         default: return "unknown status";
     }
 }
@@ -921,6 +923,51 @@ int chan_post_strain_norm(chan_t* h, int kxc, int kzc, const void* dev_db, void*
     if (rc) return rc;
     const unsigned g = (unsigned)((Q.nr * Q.npk + 127) / 128);
     PB(CHAN_KC_POST); k_post_divdiv<<<g, 128, 0, h->stream>>>(Q, (const double2*)dev_db, (double2*)dev_scratch, (double2*)dev_out, 1); LAUNCHED();
+    return CHAN_OK;
+}
+
+// ---- the one entry point that needs no caller scratch and allocates nothing ---------------------------------------------
+// chan_post_strain_norm with its scratch plane set in a file-scope device array (include/chan.h).  In host code the
+// array's name is only a stand-in for the symbol: its device address comes from cudaGetSymbolAddress, asked once per
+// device with that device current and kept in a small table.
+static __device__ __align__(256) double2 g_chan_static_scratch[CHAN_STATIC_SCRATCH_BYTES / sizeof(double2)];
+
+static int static_scratch_ptr(double2** out) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static double2* table[kMaxDev] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) return CHAN_ECUDA;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!table[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_chan_static_scratch) != cudaSuccess || !p) return CHAN_ECUDA;
+        table[dev] = (double2*)p;
+    }
+    *out = table[dev];
+    return CHAN_OK;
+}
+
+size_t chan_post_strain_norm_static_limit(void) { return (size_t)CHAN_STATIC_SCRATCH_BYTES; }
+
+int chan_post_strain_norm_static(chan_t* h, int kxc, int kzc, const void* dev_db, void* dev_out) {
+    if (!h || !dev_db || !dev_out) return CHAN_EINVAL;
+    if (!h->bound) return CHAN_ESTATE;
+    const Plan& P = h->P;
+    if (kxc < 0 || kzc < 0 || kxc > P.nxh - 1 || kzc > P.nzh - 1) return CHAN_EINVAL;
+    // one complex plane set [ny][2 kzc + 1][kxc + 1] of scratch: beyond the static array, refuse
+    if ((size_t)P.ny * (2 * kzc + 1) * (kxc + 1) * sizeof(double2) > (size_t)CHAN_STATIC_SCRATCH_BYTES) return CHAN_ELIMIT;
+    double2* scratch = nullptr;
+    int rc = static_scratch_ptr(&scratch);
+    if (rc) { h->cuda_err = (int)cudaGetLastError(); return rc; }
+    PostParams Q;
+    Q.ny = P.ny; Q.nr = 2 * kzc + 1; Q.npk = kxc + 1; Q.kzc = kzc; Q.nz = P.nz;
+    Q.B1 = h->tab[0][0]; Q.A2 = h->tab[0][1]; Q.B2 = h->tab[0][2]; Q.lu1 = h->tab[0][3];
+    Q.kx = h->kx; Q.kz = h->kz; Q.wm = h->wm; Q.wp = h->wp; Q.nu = P.nu;
+    // nothing in the scratch has to start at zero: every mode's forward sweep writes its column before the backward
+    // sweep reads it (post_d1), so the contents left by the previous call are never read
+    const unsigned g = (unsigned)((Q.nr * Q.npk + 127) / 128);
+    PB(CHAN_KC_POST); k_post_divdiv<<<g, 128, 0, h->stream>>>(Q, (const double2*)dev_db, scratch, (double2*)dev_out, 1); LAUNCHED();
     return CHAN_OK;
 }
 
