@@ -23,6 +23,11 @@
 namespace chn {
 
 #define CHAN_MAX_STAGES 8
+#ifdef __CUDA_ARCH__
+#define CHAN_ASSUME(x) __builtin_assume(x)
+#else
+#define CHAN_ASSUME(x) ((void)0)
+#endif
 
 struct FftStage {
     int R, m;              // radix, sub-block length (product of the later radices)
@@ -745,6 +750,7 @@ CHAN_HD void xpass(const XIO& io, const FftStage& S, int n, int nseq, int tid, i
         for (int w = tid; w < total; w += nt) {
             const int q = w / nb, b = w - q * nb;
             const int blk = b / m, p = b - blk * m;
+            CHAN_ASSUME(p >= 0 && p < m && blk >= 0);      // known bits: the swizzle of base + k m then folds per k
             c2 tw[R - 1];
             if (m > 1) load_twiddles<R>(S, m, p, tw);
             pass_item<R, INV, DIT>(io, io, q, blk * ncur + p, m, tw, m > 1);
@@ -776,6 +782,7 @@ CHAN_HD void xpass_any(const XIO& io, const FftStage& S, int n, int nseq, int ti
 template <int F, int NPROD>
 CHAN_HD void xfused(const XIO& io, int n, int tid, int nt) {
     for (int b = tid; b < n / F; b += nt) {
+        CHAN_ASSUME(b >= 0);
         c2 s0[F], s1[F], s2[F];
 #pragma unroll
         for (int k = 0; k < F; ++k) { s0[k] = io.load(F * b + k, 0); s1[k] = io.load(F * b + k, 1); s2[k] = io.load(F * b + k, 2); }
