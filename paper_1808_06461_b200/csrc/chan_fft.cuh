@@ -260,6 +260,7 @@ CHAN_HD void zpass(const Src& src, const Dst& dst, const FftStage& S, int n, int
     for (int w = tid; w < total; w += nt) {
         const int b = b0 + (w >> lgT), t = w & (T - 1);
         const int blk = b / m, p = b - blk * m;
+        if constexpr (M > 0) CHAN_ASSUME(p >= 0 && p < M && blk >= 0 && blk < n / (R * M));   // ranges: the truncating store folds per output
         c2 tw[R - 1 > 0 ? R - 1 : 1];
         if (m > 1) load_twiddles<R>(S, m, p, tw);
         pass_item<R, INV, DIT>(src, dst, t, blk * ncur + p, m, tw, m > 1);
@@ -555,6 +556,7 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
     ZFwdIO io = make_zfwd_io(P, T, reinterpret_cast<c2*>(smem_raw), xh + ((size_t)fi * npl + jc) * (size_t)P.mz * pin,
                              zfwd_plane(P, out.f[fi], j, filt, kxc, kzc), pin, p0, scale, filt, kxc, kzc);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
+    io.mz = mz; io.nzh = mz / 3; io.nz = 2 * (mz / 3);      // = P.mz, P.nzh, P.nz of the plan this kernel is dispatched for, as literals
     const int tid = threadIdx.x, nt = blockDim.x;
     io.gin = true;
     if constexpr (CHAN_ZASYNC && NS > 1) {
@@ -615,7 +617,9 @@ __global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
 template <int R0, int R1, int R2, int R3>
 __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
     extern __shared__ double2 smem_raw[];
-    zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, filt, kxc, kzc, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    // filt as a literal on the hot path (a3-a8 of every substep): the filter branches of the truncating store fold away
+    if (filt == 0) zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    else zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, filt, kxc, kzc, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
 }
 #endif
 
