@@ -487,6 +487,7 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
     ZInvIO io = make_zinv_io(P, T, reinterpret_cast<c2*>(smem_raw), in.f[fi] + (size_t)(j0 + jc) * P.nm,
                              zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
+    io.mz = mz; io.nzh = mz / 3; io.nz = 2 * (mz / 3);      // literals (= P.mz, P.nzh, P.nz of the plan this kernel is dispatched for)
     const int tid = threadIdx.x, nt = blockDim.x;
     if constexpr (CHAN_ZASYNC && NS > 1) {
         // retained rows s != nzh of the field -> rows e(s) of the tile; columns beyond a ragged tile are zero-filled
@@ -509,17 +510,18 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
             int lgT = 0;
             while ((1 << lgT) < T) ++lgT;
             const int t = tid & (T - 1), r0 = tid >> lgT, rs = nt >> lgT;        // nt is a multiple of 32 >= T
+            constexpr int nzh_c = mz / 3, nz_c = 2 * (mz / 3);                     // literals, as above
             const bool live = t < io.tcount;
             const double2* g = io.src + (size_t)r0 * P.nxh + p0 + t;
             c2* d = sm + r0 * T + t;
             const size_t gs = (size_t)rs * P.nxh;
             const int ds = rs * T;
 #pragma unroll 4
-            for (int sl = r0; sl < P.nzh; sl += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
-            g = io.src + (size_t)(P.nzh + 1 + r0) * P.nxh + p0 + t;
-            d = sm + (P.nzh + 1 + r0 + (mz - P.nz)) * T + t;
+            for (int sl = r0; sl < nzh_c; sl += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
+            g = io.src + (size_t)(nzh_c + 1 + r0) * P.nxh + p0 + t;
+            d = sm + (nzh_c + 1 + r0 + (mz - nz_c)) * T + t;
 #pragma unroll 4
-            for (int sl = P.nzh + 1 + r0; sl < P.nz; sl += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
+            for (int sl = nzh_c + 1 + r0; sl < nz_c; sl += rs, g += gs, d += ds) { if (live) cp_async16(d, g); else *d = mk(0, 0); }
             cp_async_wait_all();
         }
         __syncthreads();
