@@ -479,9 +479,13 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.com
 
 // Bodies with explicit block coordinates (bx = column tile, jc = plane of the chunk, fi = field), shared by the
 // stand-alone kernels below and by the merged plane kernel k_planes_s.
-template <int R0, int R1, int R2, int R3>
-__device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs& in, int j0, int npl, double2* __restrict__ zpad, int T,
+// default columns per z tile for a transform length (the rule of choose_tiling in chan_api.cu): the specialised kernels
+// take that T as a literal (TC), so that tile addresses become one base plus immediates; any other T runs with TC = 0
+__host__ __device__ constexpr int ztile_default(int mz) { int T = 16; while (T > 1 && (long)mz * T * 16 > 112 * 1024) T >>= 1; return T; }
+template <int R0, int R1, int R2, int R3, int TC = 0>
+__device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs& in, int j0, int npl, double2* __restrict__ zpad, int Trt,
                                           double2* smem_raw, int bx, int jc, int fi) {
+    const int T = TC > 0 ? TC : Trt;
     constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
     const int p0 = bx * T;
     ZInvIO io = make_zinv_io(P, T, reinterpret_cast<c2*>(smem_raw), in.f[fi] + (size_t)(j0 + jc) * P.nm,
@@ -549,9 +553,10 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
         zpass<R3, true, false, 1>(io, io, P.fz.st[3], mz, T, tid, nt);
     }
 }
-template <int R0, int R1, int R2, int R3>
+template <int R0, int R1, int R2, int R3, int TC = 0>
 __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* __restrict__ xh, int pin, int j0, int npl, const FieldPtrsW& out,
-                                          double scale, int filt, int kxc, int kzc, int T, double2* smem_raw, int bx, int jc, int fi) {
+                                          double scale, int filt, int kxc, int kzc, int Trt, double2* smem_raw, int bx, int jc, int fi) {
+    const int T = TC > 0 ? TC : Trt;
     constexpr int NS = (R0 > 1) + (R1 > 1) + (R2 > 1) + (R3 > 1);
     const int p0 = bx * T;
     const int j = j0 + jc;
@@ -614,13 +619,17 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
 template <int R0, int R1, int R2, int R3>
 __global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
     extern __shared__ double2 smem_raw[];
-    zinv_body<R0, R1, R2, R3>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    constexpr int TD = ztile_default(R0 * R1 * R2 * R3);
+    if (T == TD) zinv_body<R0, R1, R2, R3, TD>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    else zinv_body<R0, R1, R2, R3>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
 }
 template <int R0, int R1, int R2, int R3>
 __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
     extern __shared__ double2 smem_raw[];
     // filt as a literal on the hot path (a3-a8 of every substep): the filter branches of the truncating store fold away
-    if (filt == 0) zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    constexpr int TD = ztile_default(R0 * R1 * R2 * R3);
+    if (filt == 0 && T == TD) zfwd_body<R0, R1, R2, R3, TD>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    else if (filt == 0) zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
     else zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, filt, kxc, kzc, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
 }
 #endif
