@@ -948,7 +948,10 @@ __device__ __forceinline__ void xprod_body(const PlaneParams& P, const double2* 
     const int tid = threadIdx.x, nt = blockDim.x;
     XIO io; io.sm = reinterpret_cast<c2*>(smem_raw); io.stride = mx;
     io.blo = mx / 3; io.bhi = mx - mx / 3;
-    xpack(io, mx, P.nxh, zpad + ((size_t)jc * P.mz + r) * P.nxh, (size_t)npl * P.mz * P.nxh, tid, nt, R0 == 1);
+    // P.nxh of the plan this kernel is dispatched for, as a literal in the substep's kernel (the filter variant, at its 128-register
+    // cap with a spill, got 5% slower with it and keeps the run-time value)
+    const int nxh = NPROD == 3 ? mx / 3 : P.nxh;
+    xpack(io, mx, nxh, zpad + ((size_t)jc * P.mz + r) * nxh, (size_t)npl * P.mz * nxh, tid, nt, R0 == 1);
     __syncthreads();
     if constexpr (R0 > 1) { io.zin = true; xpass<R0, true, false, M0>(io, P.fx.st[0], mx, 3, tid, nt); io.zin = false; __syncthreads(); }
     if constexpr (R1 > 1) { xpass<R1, true, false, M1>(io, P.fx.st[1], mx, 3, tid, nt); __syncthreads(); }
@@ -958,7 +961,8 @@ __device__ __forceinline__ void xprod_body(const PlaneParams& P, const double2* 
     if constexpr (R2 > 1) { xpass<R2, false, true, M2>(io, P.fx.st[2], mx, NC, tid, nt); __syncthreads(); }
     if constexpr (R1 > 1) { xpass<R1, false, true, M1>(io, P.fx.st[1], mx, NC, tid, nt); __syncthreads(); }
     if constexpr (R0 > 1) { io.zout = true; xpass<R0, false, true, M0>(io, P.fx.st[0], mx, NC, tid, nt); io.zout = false; __syncthreads(); }
-    xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
+    if (NPROD == 3 && pout == nxh) xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * nxh, (size_t)npl * P.mz * nxh, nxh, tid, nt);
+    else xunpack<NPROD>(io, mx, xh + ((size_t)jc * P.mz + r) * pout, (size_t)npl * P.mz * pout, pout, tid, nt);
 }
 #ifndef CHAN_XNT
 #define CHAN_XNT 256      // most threads of an x-pass CTA (two CTAs per SM)
