@@ -940,12 +940,12 @@ __global__ void __launch_bounds__(256, 2) k_xfft_prod_g(CHAN_XARGS) {
 
 // stage radices as template parameters: R0, R1, R2 (1 = absent) then the fused radix F
 // (the filter variant keeps four sequences in shared memory: where only one such CTA fits on an SM it runs 512 threads)
-template <int NPROD, int F, int R0, int R1, int R2>
+template <int NPROD, int F, int R0, int R1, int R2, int NTC = 0>
 __device__ __forceinline__ void xprod_body(const PlaneParams& P, const double2* __restrict__ zpad, int npl, double2* __restrict__ xh, int pout,
                                            double2* smem_raw, int r, int jc) {
     constexpr int NC = (NPROD + 1) / 2;
     constexpr int M2 = F, M1 = R2 * F, M0 = R1 * R2 * F, mx = R0 * M0;
-    const int tid = threadIdx.x, nt = blockDim.x;
+    const int tid = threadIdx.x, nt = NTC > 0 ? NTC : blockDim.x;      // NTC: the CTA size as a literal (trip counts of the item loops fold)
     XIO io; io.sm = reinterpret_cast<c2*>(smem_raw); io.stride = mx;
     io.blo = mx / 3; io.bhi = mx - mx / 3;
     // P.nxh of the plan this kernel is dispatched for, as a literal in the substep's kernel (the filter variant, at its 128-register
@@ -970,7 +970,9 @@ __device__ __forceinline__ void xprod_body(const PlaneParams& P, const double2* 
 template <int NPROD, int F, int R0, int R1, int R2>
 __global__ void __launch_bounds__(NPROD == 7 ? 512 : CHAN_XNT, NPROD == 7 ? 1 : 2) k_xfft_prod_s(CHAN_XARGS) {
     extern __shared__ double2 smem_raw[];
-    xprod_body<NPROD, F, R0, R1, R2>(P, zpad, npl, xh, pout, smem_raw, blockIdx.x, blockIdx.y);
+    // (the same for 128-thread CTAs, as configs 3 and 4 run them, was measured 7% slower and is not dispatched)
+    if (NPROD == 3 && blockDim.x == 256) xprod_body<NPROD, F, R0, R1, R2, 256>(P, zpad, npl, xh, pout, smem_raw, blockIdx.x, blockIdx.y);
+    else xprod_body<NPROD, F, R0, R1, R2>(P, zpad, npl, xh, pout, smem_raw, blockIdx.x, blockIdx.y);
 }
 
 // =====================================================================================================
