@@ -482,7 +482,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.com
 // default columns per z tile for a transform length (the rule of choose_tiling in chan_api.cu): the specialised kernels
 // take that T as a literal (TC), so that tile addresses become one base plus immediates; any other T runs with TC = 0
 __host__ __device__ constexpr int ztile_default(int mz) { int T = 16; while (T > 1 && (long)mz * T * 16 > 112 * 1024) T >>= 1; return T; }
-template <int R0, int R1, int R2, int R3, int TC = 0>
+template <int R0, int R1, int R2, int R3, int TC = 0, int NTC = 0>
 __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs& in, int j0, int npl, double2* __restrict__ zpad, int Trt,
                                           double2* smem_raw, int bx, int jc, int fi) {
     const int T = TC > 0 ? TC : Trt;
@@ -492,7 +492,7 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
                              zpad + ((size_t)fi * npl + jc) * (size_t)P.mz * P.nxh, p0);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     io.mz = mz; io.nzh = mz / 3; io.nz = 2 * (mz / 3);      // literals (= P.mz, P.nzh, P.nz of the plan this kernel is dispatched for)
-    const int tid = threadIdx.x, nt = blockDim.x;
+    const int tid = threadIdx.x, nt = NTC > 0 ? NTC : blockDim.x;
     if constexpr (CHAN_ZASYNC && NS > 1) {
         // retained rows s != nzh of the field -> rows e(s) of the tile; columns beyond a ragged tile are zero-filled
         c2* sm = io.sm;
@@ -553,7 +553,7 @@ __device__ __forceinline__ void zinv_body(const PlaneParams& P, const FieldPtrs&
         zpass<R3, true, false, 1>(io, io, P.fz.st[3], mz, T, tid, nt);
     }
 }
-template <int R0, int R1, int R2, int R3, int TC = 0>
+template <int R0, int R1, int R2, int R3, int TC = 0, int NTC = 0>
 __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* __restrict__ xh, int pin, int j0, int npl, const FieldPtrsW& out,
                                           double scale, int filt, int kxc, int kzc, int Trt, double2* smem_raw, int bx, int jc, int fi) {
     const int T = TC > 0 ? TC : Trt;
@@ -564,7 +564,7 @@ __device__ __forceinline__ void zfwd_body(const PlaneParams& P, const double2* _
                              zfwd_plane(P, out.f[fi], j, filt, kxc, kzc), pin, p0, scale, filt, kxc, kzc);
     constexpr int M2 = R3, M1 = R2 * R3, M0 = R1 * R2 * R3, mz = R0 * M0;
     io.mz = mz; io.nzh = mz / 3; io.nz = 2 * (mz / 3);      // = P.mz, P.nzh, P.nz of the plan this kernel is dispatched for, as literals
-    const int tid = threadIdx.x, nt = blockDim.x;
+    const int tid = threadIdx.x, nt = NTC > 0 ? NTC : blockDim.x;
     io.gin = true;
     if constexpr (CHAN_ZASYNC && NS > 1) {
         c2* sm = io.sm;
@@ -620,7 +620,8 @@ template <int R0, int R1, int R2, int R3>
 __global__ void __launch_bounds__(256, 2) k_zfft_inv_s(CHAN_ZARGS_INV) {
     extern __shared__ double2 smem_raw[];
     constexpr int TD = ztile_default(R0 * R1 * R2 * R3);
-    if (T == TD) zinv_body<R0, R1, R2, R3, TD>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    if (T == TD && blockDim.x == 192) zinv_body<R0, R1, R2, R3, TD, 192>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    else if (T == TD) zinv_body<R0, R1, R2, R3, TD>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
     else zinv_body<R0, R1, R2, R3>(P, in, j0, npl, zpad, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
 }
 template <int R0, int R1, int R2, int R3>
@@ -628,7 +629,8 @@ __global__ void __launch_bounds__(256, 2) k_zfft_fwd_s(CHAN_ZARGS_FWD) {
     extern __shared__ double2 smem_raw[];
     // filt as a literal on the hot path (a3-a8 of every substep): the filter branches of the truncating store fold away
     constexpr int TD = ztile_default(R0 * R1 * R2 * R3);
-    if (filt == 0 && T == TD) zfwd_body<R0, R1, R2, R3, TD>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    if (filt == 0 && T == TD && blockDim.x == 192) zfwd_body<R0, R1, R2, R3, TD, 192>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
+    else if (filt == 0 && T == TD) zfwd_body<R0, R1, R2, R3, TD>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
     else if (filt == 0) zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, 0, 0, 0, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
     else zfwd_body<R0, R1, R2, R3>(P, xh, pin, j0, npl, out, scale, filt, kxc, kzc, T, smem_raw, blockIdx.x, blockIdx.y, blockIdx.z);
 }
