@@ -91,6 +91,9 @@ template <int R> __device__ __forceinline__ double band7r(const double* c, const
     for (int k = 1; k < 7; ++k) s += c[k] * w[(R + 1 + k) % 7];
     return s;
 }
+// a chunk of YR iterations it0 .. it0+YR-1 whose rows are all interior for every index a sweep forms from them: the trailing
+// row (iteration - 3) is past the first wall, and the row CHAN_PF ahead of the last iteration still exists
+__device__ __forceinline__ bool interior_chunk(int it0, int ny) { return it0 >= YR && it0 + YR + CHAN_PF <= ny; }
 struct Rec3 { double x[3]; __device__ __forceinline__ void init() { x[0] = x[1] = x[2] = 0.0; } };
 // back substitution with a factor row f = {1/d, u1, u2, u3}
 template <int R> __device__ __forceinline__ double bwd3(Rec3& s, double4 f, double z) {
@@ -501,16 +504,19 @@ __global__ void __launch_bounds__(YNT, 6) k_se(YParams P, double2* zv_zu, const 
         stage8n(sLUb, P.t[1].lu1, ny, it0, ny - 1, -1, YR);  // back substitution of the orientation-1 system: virtual row ny-1-jj
         stage8n(sB1, P.t[0].B1, ny, it0, -3, 1, YR); stage8n(sLU, P.t[0].lu1, ny, it0, -3, 1, YR);
         __syncthreads();
-        static_for<YR>([&](auto ic) {
+        // IN: every row of this chunk is an interior row (no wall, nothing beyond either end within the prefetch distance):
+        // the per-row range checks fold away (the sweeps issue 40-60% of their slots, most of it index and predicate work)
+        auto row = [&](auto ic, auto interior) {
             constexpr int R = decltype(ic)::value;
+            constexpr bool IN = decltype(interior)::value;
             const int jj = it0 + R;
-            if (jj < nit) {
+            if (IN || jj < nit) {
                 double a = 0.0, b = 0.0;
-                const bool ld = S.act && jj < ny;
+                const bool ld = S.act && (IN || jj < ny);
                 if (ld) {
-                    if (jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(zv_zu + op); pf2(omy + op); }
+                    if (IN || jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(zv_zu + op); pf2(omy + op); }
                     const double zvv = nzv, oy = noy;
-                    if (jj + 1 < ny) { nzv = *cpart(zv_zu, ol + nm, part); noy = *cpart(omy, ol + nm, part); }   // next row, one step ahead
+                    if (IN || jj + 1 < ny) { nzv = *cpart(zv_zu, ol + nm, part); noy = *cpart(omy, ol + nm, part); }   // next row, one step ahead
                     const double dv = d1bwd3<R>(bs, sLUb + R * 8, zvv);
                     a = S.kx * dv - S.kz * oy;
                     b = S.kz * dv + S.kx * oy;
@@ -519,17 +525,19 @@ __global__ void __launch_bounds__(YNT, 6) k_se(YParams P, double2* zv_zu, const 
                 const double oa = __shfl_xor_sync(0xffffffffu, a, 1), ob = __shfl_xor_sync(0xffffffffu, b, 1);
                 double uj = 0.0, wj = 0.0;
                 if (ld) { uj = (part ? oa : -oa) * rk2; wj = (part ? ob : -ob) * rk2; }
-                if (mean && jj < ny && part == 0) { uj = __ldg(U + jj); wj = __ldg(W + jj); }
-                if (wr && jj < ny) { *wpart(u, ol, part) = uj; *wpart(w_, ol, part) = wj; }
+                if (mean && (IN || jj < ny) && part == 0) { uj = __ldg(U + jj); wj = __ldg(W + jj); }
+                if (wr && (IN || jj < ny)) { *wpart(u, ol, part) = uj; *wpart(w_, ol, part) = wj; }
                 wu[R % 7] = uj; ww[R % 7] = wj;
-                if (wr && jj >= 3) {
+                if (wr && (IN || jj >= 3)) {
                     const size_t oc = ol - 3 * nm;
                     *wpart(zv_zu, oc, part) = d1fwd3<R>(fu, sLU + R * 8, band7r<R>(sB1 + R * 8, wu));
                     *wpart(zw, oc, part) = d1fwd3<R>(fw, sLU + R * 8, band7r<R>(sB1 + R * 8, ww));
                 }
                 ol += nm;
             }
-        });
+        };
+        if (interior_chunk(it0, ny)) static_for<YR>([&](auto ic) { row(ic, std::true_type{}); });
+        else static_for<YR>([&](auto ic) { row(ic, std::false_type{}); });
     }
 }
 
