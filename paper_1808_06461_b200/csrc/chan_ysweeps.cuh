@@ -152,6 +152,12 @@ __device__ __forceinline__ void helm_row_s(int ny, int i, double lam, const doub
     }
 }
 
+template <bool IN> __device__ __forceinline__ void helm_row_t(int ny, int i, double lam, const double* a2, const double* b2, double (&a)[7]) {
+    if constexpr (IN) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) a[k] = b2[k] - lam * a2[k];
+    } else helm_row_s(ny, i, lam, a2, b2, a);
+}
 __device__ __forceinline__ const double* cpart(const double2* a, size_t o, int part) { return reinterpret_cast<const double*>(a + o) + part; }
 __device__ __forceinline__ double* wpart(double2* a, size_t o, int part) { return reinterpret_cast<double*>(a + o) + part; }
 
@@ -178,13 +184,14 @@ __global__ void __launch_bounds__(YNT) k_sa(YParams P, const double2* __restrict
         stage8n(sB1, P.t[0].B1, ny, it0, -3, 1, YR); stage8n(sLU, P.t[0].lu1, ny, it0, -3, 1, YR);
         stage8n(sA2, P.t[0].A2, ny, it0, -3, 1, YR); stage8n(sB2, P.t[0].B2, ny, it0, -3, 1, YR);
         __syncthreads();
-        static_for<YR>([&](auto ic) {
+        auto row = [&](auto ic, auto interior) {      // IN: a chunk of interior rows, the range checks fold (see k_se)
             constexpr int R = decltype(ic)::value;
+            constexpr bool IN = decltype(interior)::value;
             const int jj = it0 + R;
-            if (jj < nit) {
+            if (IN || jj < nit) {
                 double d = 0.0, x = 0.0, t = 0.0;
-                if (S.act && jj < ny) {
-                    if (jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(H1 + op); pf2(H3 + op); pf2(omy + op); if (hist) pf2(hg + op); }
+                if (S.act && (IN || jj < ny)) {
+                    if (IN || jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(H1 + op); pf2(H3 + op); pf2(omy + op); if (hist) pf2(hg + op); }
                     const c2 h1 = ldc(H1 + ol), h3 = ldc(H3 + ol);
                     x = *cpart(omy, ol, part);
                     const double gp = hist ? *cpart(hg, ol, part) : 0.0;     // zeta_1 = 0: the first substep reads no history
@@ -196,11 +203,11 @@ __global__ void __launch_bounds__(YNT) k_sa(YParams P, const double2* __restrict
                 }
                 wd[R % 7] = d; wx[R % 7] = x; wt[R % 7] = t;
                 const int j = jj - 3;
-                if (S.act && j >= 0) {
+                if (S.act && (IN || j >= 0)) {
                     const size_t oc = ol - 3 * nm;
                     *wpart(zd, oc, part) = d1fwd3<R>(fd, sLU + R * 8, band7r<R>(sB1 + R * 8, wd));
                     double r = 0.0;
-                    if (j != 0 && j != ny - 1) {
+                    if (IN || (j != 0 && j != ny - 1)) {
                         const double at = band7r<R>(sA2 + R * 8, wt), bx = band7r<R>(sB2 + R * 8, wx), ax = band7r<R>(sA2 + R * 8, wx);
                         r = -c * (at + P.alpha * P.nu * P.dt * (bx - S.k2 * ax));
                     }
@@ -208,7 +215,9 @@ __global__ void __launch_bounds__(YNT) k_sa(YParams P, const double2* __restrict
                 }
                 ol += nm;
             }
-        });
+        };
+        // (the interior-chunk variant cost this sweep 20 registers and a CTA per SM: measured slower, not dispatched)
+        static_for<YR>([&](auto ic) { row(ic, std::false_type{}); });
     }
 }
 
@@ -241,33 +250,34 @@ __global__ void __launch_bounds__(YNT, 4) k_sb(YParams P, const double2* __restr
         stage8n(sLU, P.t[0].lu1, ny, it0, ny - 1, -1, YR);        // orientation-0 LU of A1 at physical row j = ny-1-ii
         stage8n(sA2, P.t[1].A2, ny, it0, -3, 1, YR); stage8n(sB2, P.t[1].B2, ny, it0, -3, 1, YR);   // orientation 1, virtual row i = ii-3
         __syncthreads();
-        static_for<YR>([&](auto ic) {
+        auto row = [&](auto ic, auto interior) {      // IN: a chunk of interior rows, the range checks fold (see k_se)
             constexpr int R = decltype(ic)::value;
+            constexpr bool IN = decltype(interior)::value;
             const int ii = it0 + R;
-            if (ii < nit) {
+            if (IN || ii < nit) {
                 const int j = ny - 1 - ii;
                 const int i = ii - 3;
                 double x = 0.0, t = 0.0, romv = 0.0;
                 const size_t oc = (size_t)(ol + 3 * (long long)nm);     // row ny-1-i = j+3
-                if (S.act && i >= 0) romv = *cpart(rom_zom, oc, part);
-                if (S.act && j >= 0) {
+                if (S.act && (IN || i >= 0)) romv = *cpart(rom_zom, oc, part);
+                if (S.act && (IN || j >= 0)) {
                     const size_t o = (size_t)ol;
-                    if (j - CHAN_PF >= 0) { const size_t op = o - (size_t)CHAN_PF * nm; pf2(zd_zphi + op); pf2(H2 + op); pf2(phi + op); if (hist) pf2(hv + op); pf2(rom_zom + op); }
+                    if (IN || j - CHAN_PF >= 0) { const size_t op = o - (size_t)CHAN_PF * nm; pf2(zd_zphi + op); pf2(H2 + op); pf2(phi + op); if (hist) pf2(hv + op); pf2(rom_zom + op); }
                     const double zdv = nzd, h2 = nh2, hp = nhp;
                     x = nph;
-                    if (j > 0) { const size_t o1 = o - nm; nzd = *cpart(zd_zphi, o1, part); nh2 = *cpart(H2, o1, part); nhp = hist ? *cpart(hv, o1, part) : 0.0; nph = *cpart(phi, o1, part); }
+                    if (IN || j > 0) { const size_t o1 = o - nm; nzd = *cpart(zd_zphi, o1, part); nh2 = *cpart(H2, o1, part); nhp = hist ? *cpart(hv, o1, part) : 0.0; nph = *cpart(phi, o1, part); }
                     const double dd = d1bwd3<R>(bd, sLU + R * 8, zdv);
                     const double h = -S.k2 * h2 - dd;
                     *wpart(hv, o, part) = h;
                     t = x + P.dt * (P.gamma * h + P.zeta * hp);
                 }
                 wx[R % 7] = x; wt[R % 7] = t;
-                if (S.act && i >= 0) {
+                if (S.act && (IN || i >= 0)) {
                     const double* a2 = sA2 + R * 8; const double* b2 = sB2 + R * 8;
                     double a[7];
-                    helm_row_s(ny, i, lam, a2, b2, a);
+                    helm_row_t<IN>(ny, i, lam, a2, b2, a);
                     double r = 0.0;
-                    if (i != 0 && i != ny - 1) {
+                    if (IN || (i != 0 && i != ny - 1)) {
                         const double at = band7r<R>(a2, wt), bx = band7r<R>(b2, wx), ax = band7r<R>(a2, wx);
                         r = -c * (at + P.alpha * P.nu * P.dt * (bx - S.k2 * ax));
                     }
@@ -275,11 +285,13 @@ __global__ void __launch_bounds__(YNT, 4) k_sb(YParams P, const double2* __restr
                     *wpart(zd_zphi, oc, part) = hf.template fwd<R>(rz, r);
                     *wpart(rom_zom, oc, part) = hf.template fwd<R>(ro, romv);
                     if (part == 0) facA[oc] = make_double2(f.x, f.y);
-                    else facB[oc] = make_double2(f.z, hf.template fwd<R>(rb, i == 0 ? 1.0 : 0.0));   // virtual row 0 = wall y=+1
+                    else facB[oc] = make_double2(f.z, hf.template fwd<R>(rb, (!IN && i == 0) ? 1.0 : 0.0));   // virtual row 0 = wall y=+1
                 }
                 ol -= (long long)nm;
             }
-        });
+        };
+        // (the interior-chunk variant cost this sweep 20 registers and a CTA per SM: measured slower, not dispatched)
+        static_for<YR>([&](auto ic) { row(ic, std::false_type{}); });
     }
 }
 
@@ -315,35 +327,36 @@ __global__ void __launch_bounds__(YNT) k_sc(YParams P, double2* facA, double2* f
         stage1n(sWm, P.wm, ny, it0, -3, 1, YR, 0, 1); stage1n(sWp, P.wp, ny, it0, -3, 1, YR, 0, 1);
         stage1n(sA6, P.t[1].A2, ny, it0, ny - 1, -1, YR, 6, 8); stage1n(sB6, P.t[1].B2, ny, it0, ny - 1, -1, YR, 6, 8);   // virtual row ny-1-jj
         __syncthreads();
-        static_for<YR>([&](auto ic) {
+        auto row = [&](auto ic, auto interior) {      // IN: a chunk of interior rows, the range checks fold (see k_se)
             constexpr int R = decltype(ic)::value;
+            constexpr bool IN = decltype(interior)::value;
             const int jj = it0 + R;
-            if (jj < nit) {
+            if (IN || jj < nit) {
                 double pp = 0.0, pab = 0.0;
-                if (S.act && jj < ny) {
-                    if (jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(facA + op); pf2(facB + op); pf2(zom_zvab + op); pf2(zphi_phip + op); }
+                if (S.act && (IN || jj < ny)) {
+                    if (IN || jj + CHAN_PF < ny) { const size_t op = ol + (size_t)CHAN_PF * nm; pf2(facA + op); pf2(facB + op); pf2(zom_zvab + op); pf2(zphi_phip + op); }
                     const double2 fa = nfa, fb = nfb;
                     const double zo = nzo, zp = nzp;
-                    if (jj + 1 < ny) { const size_t o1 = ol + nm; nfa = facA[o1]; nfb = facB[o1]; nzo = *cpart(zom_zvab, o1, part); nzp = *cpart(zphi_phip, o1, part); }
+                    if (IN || jj + 1 < ny) { const size_t o1 = ol + nm; nfa = facA[o1]; nfb = facB[o1]; nzo = *cpart(zom_zvab, o1, part); nzp = *cpart(zphi_phip, o1, part); }
                     const int iv = ny - 1 - jj;
-                    const double u3 = (iv == 0 || iv == ny - 1) ? 0.0 : sB6[R] - lam * sA6[R];
+                    const double u3 = (!IN && (iv == 0 || iv == ny - 1)) ? 0.0 : sB6[R] - lam * sA6[R];
                     const double4 f = make_double4(fa.x, fa.y, fb.x, u3);
                     *wpart(omy, ol, part) = bwd3<R>(bo, f, zo);
                     pp = bwd3<R>(bp, f, zp);
                     // problem a: phi(-1) = 1, its forward-eliminated right-hand side is the unit vector at the last
                     // virtual row (physical row 0); problem b: phi(+1) = 1, z_b from SB
-                    pab = bwd3<R>(bab, f, part ? fb.y : (jj == 0 ? 1.0 : 0.0));
+                    pab = bwd3<R>(bab, f, part ? fb.y : ((!IN && jj == 0) ? 1.0 : 0.0));
                     *wpart(zphi_phip, ol, part) = pp;
                     *wpart(phiab, ol, part) = pab;
                 }
                 wp_[R % 7] = pp; wab[R % 7] = pab;
                 const int j = jj - 3;
-                if (S.act && j >= 0) {
+                if (S.act && (IN || j >= 0)) {
                     const size_t oc = ol - 3 * nm;
                     const double* a2 = sA2 + R * 8;
                     double a[7];
-                    helm_row_s(ny, j, S.k2, a2, sB2 + R * 8, a);
-                    const bool wall = (j == 0 || j == ny - 1);
+                    helm_row_t<IN>(ny, j, S.k2, a2, sB2 + R * 8, a);
+                    const bool wall = !IN && (j == 0 || j == ny - 1);
                     const double r = wall ? 0.0 : band7r<R>(a2, wp_), rr = wall ? 0.0 : band7r<R>(a2, wab);
                     // adjoint recurrence with the rows j-1, j-2, j-3 of U still in hf
                     const double tm = sWm[R] - hf.u1[(R + 2) % 3] * gm.x[(R + 2) % 3] - hf.u2[(R + 1) % 3] * gm.x[(R + 1) % 3] - hf.u3[R % 3] * gm.x[R % 3];
@@ -362,7 +375,10 @@ __global__ void __launch_bounds__(YNT) k_sc(YParams P, double2* facA, double2* f
                 __syncwarp();
                 ol += nm;
             }
-        });
+        };
+        // (the interior-chunk variant pushed this sweep past the 168 registers that let three CTAs share an SM, and was slower
+        // under that cap as well: not dispatched)
+        static_for<YR>([&](auto ic) { row(ic, std::false_type{}); });
     }
     // influence matrix (step 7): G = [[w-.v_a, w-.v_b],[w+.v_a, w+.v_b]], (c_a, c_b) = -G^-1 (w-.v_p, w+.v_p)
     const double oabm = __shfl_xor_sync(0xffffffffu, sabm, 1), oabp = __shfl_xor_sync(0xffffffffu, sabp, 1);
@@ -407,22 +423,23 @@ __global__ void __launch_bounds__(YNT) k_sd(YParams P, const double2* __restrict
         __syncthreads();
         stage8n(sB1, P.t[1].B1, ny, it0, -3, 1, YR); stage8n(sLU, P.t[1].lu1, ny, it0, -3, 1, YR);
         __syncthreads();
-        static_for<YR>([&](auto ic) {
+        auto row = [&](auto ic, auto interior) {      // IN: a chunk of interior rows, the range checks fold (see k_se)
             constexpr int R = decltype(ic)::value;
+            constexpr bool IN = decltype(interior)::value;
             const int ii = it0 + R;
-            if (ii < nit) {
+            if (IN || ii < nit) {
                 const int j = ny - 1 - ii;
                 double v = 0.0;
                 // each lane reads only the slot of phi_ab / z_vab it owns (and later overwrites); the partner's
                 // value comes by shuffle, so the in-place update of phi_ab by v is free of read/write hazards
-                const bool on = S.act && j >= 0;
+                const bool on = S.act && (IN || j >= 0);
                 const size_t o = on ? (size_t)ol : 0;
                 double myz = 0.0, myp = 0.0, zp = 0.0, pp = 0.0;
                 double2 fa = make_double2(1.0, 0.0), fb = make_double2(0.0, 0.0);
                 if (on) {
-                    if (j - CHAN_PF >= 0) { const size_t op = o - (size_t)CHAN_PF * nm; pf2(facA + op); pf2(facB + op); pf2(zvp + op); pf2(zvab + op); pf2(phip_zv + op); pf2(phiab_v + op); }
+                    if (IN || j - CHAN_PF >= 0) { const size_t op = o - (size_t)CHAN_PF * nm; pf2(facA + op); pf2(facB + op); pf2(zvp + op); pf2(zvab + op); pf2(phip_zv + op); pf2(phiab_v + op); }
                     myz = nmyz; myp = nmyp; fa = nfa; fb = nfb; zp = nzp; pp = npp;
-                    if (j > 0) {
+                    if (IN || j > 0) {
                         const size_t o1 = o - nm;
                         nmyz = *cpart(zvab, o1, part); nmyp = *cpart(phiab_v, o1, part); nfa = facA[o1]; nfb = facB[o1];
                         nzp = *cpart(zvp, o1, part); npp = *cpart(phip_zv, o1, part);
@@ -436,11 +453,13 @@ __global__ void __launch_bounds__(YNT) k_sd(YParams P, const double2* __restrict
                     *wpart(phi, o, part) = pp + ca * pa + cb * pb;
                 }
                 wv[R % 7] = v;
-                if (S.act && ii >= 3)
+                if (S.act && (IN || ii >= 3))
                     *wpart(phip_zv, (size_t)(ol + 3 * (long long)nm), part) = d1fwd3<R>(fw, sLU + R * 8, band7r<R>(sB1 + R * 8, wv));
                 ol -= (long long)nm;
             }
-        });
+        };
+        if (interior_chunk(it0, ny)) static_for<YR>([&](auto ic) { row(ic, std::true_type{}); });
+        else static_for<YR>([&](auto ic) { row(ic, std::false_type{}); });
     }
 }
 
