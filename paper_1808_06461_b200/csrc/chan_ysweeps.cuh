@@ -35,7 +35,10 @@
 
 namespace chn {
 
-constexpr int YNT = 128;    // threads per CTA = 64 modes
+#ifndef CHAN_YNT
+#define CHAN_YNT 128
+#endif
+constexpr int YNT = CHAN_YNT;    // threads per CTA (two per mode): 128 = 64 modes
 
 struct YS {                 // per-thread identity
     long long m;            // mode
