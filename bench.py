@@ -480,6 +480,12 @@ def main():
         if gms > 0:
             gb = bpp * npts * 3 * K / (gms * 1e-3) / 1e9     # substep part only: the filter has its own classes
             groups[gname] = {"ms_per_substep": gms / (3 * K), "survey_bytes_per_point": bpp, "achieved_GBs": gb, "frac": gb / peak}
+            if gname.startswith("K5+K1"):
+                # the six sweeps move 384 B/point (the intermediates between dependent solves); the fraction
+                # on those bytes says how close the sweeps themselves are to the roof, the one on 144 how far the design is
+                moved = sum(BYTES_PER_POINT[k] for k in ("y1", "y2", "y3", "y4", "derive_down", "derive_up"))
+                groups[gname]["moved_bytes_per_point"] = moved
+                groups[gname]["frac_on_moved_bytes"] = moved * npts * 3 * K / (gms * 1e-3) / 1e9 / peak
     sub_gb = 432 * npts / (ms_sub / (3 * K) * 1e-3) / 1e9    # 54 field passes = 432 B/point per substep
     groups["substep total"] = {"ms_per_substep": ms_sub / (3 * K), "survey_bytes_per_point": 432, "achieved_GBs": sub_gb, "frac": sub_gb / peak}
     kernel_ms = {k: {"ms_per_step": v_[0] / K, "launches_per_step": v_[1] / K} for k, v_ in sub_classes.items()}
